@@ -1,0 +1,205 @@
+/*
+ * dedisp.h -- C ABI of the B200 (sm_100a) incoherent de-dispersion library.
+ *
+ * The operation is the hot path of Magro et al., "Real-time, fast radio transient searches with
+ * GPU de-dispersion" (arXiv 1107.2516); citations are PAPER.md:<line>.
+ *
+ *   brute force   out[d][t] = sum_c in[c][t + shift(c,d)]
+ *   shift(c,d)    = round(4.15e6 ms * (f_c^-2 - f_top^-2) * DM_d / t_samp)  (eq. 1)
+ *   two-stage     sub[k][s][t] = sum_{c in subband s} in[c][t + s1(c,k)]
+ *                 out[d][t]    = sum_s sub[k(d)][s][t + s2(d,s)]
+ *   streaming     the last max_delay samples of every channel are carried from one chunk to
+ *                 the next ("n_samp + maxshift" samples per buffer)
+ *
+ * Conventions
+ *   - Plain C types only.  Every pointer is marked HOST or DEVICE.  DEVICE pointers are CUDA
+ *     device pointers of the current device, owned by the caller; the library never frees or
+ *     reallocates them.  Plans, their device tables, the subband scratch and the streaming carry
+ *     buffers are owned by the library and released by the matching *_destroy.
+ *   - Data layout: input is channel-major and time-contiguous, channel 0 is the
+ *     highest frequency f_top, channel c is at f_top - c*df.  Batches ("beams") are outermost.
+ *   - dedisp_execute / dedisp_stream_push enqueue work on the given cudaStream_t and return
+ *     without synchronising.  Argument errors are reported synchronously; a CUDA launch error
+ *     is reported as DEDISP_ECUDA by the call that saw it.
+ *   - No exceptions cross this boundary, nothing calls exit(), there is no global state.
+ *   - There is no CPU fallback: without a CUDA device every execute/push returns DEDISP_ECUDA.
+ *     Plan creation and the table getters are host-only and work without a device.
+ */
+#ifndef DEDISP_H
+#define DEDISP_H
+
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define DEDISP_API __attribute__((visibility("default")))
+#else
+#define DEDISP_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dedisp_plan dedisp_plan;     /* opaque, library-owned */
+typedef struct dedisp_stream dedisp_stream; /* opaque, library-owned */
+
+typedef enum {
+    DEDISP_OK = 0,
+    DEDISP_EINVAL = 1, /* bad scalar argument / NULL pointer / bad DM list               */
+    DEDISP_ENOMEM = 2, /* host or device allocation failed                                */
+    DEDISP_ECUDA = 3,  /* CUDA runtime error (no device, launch failure, ...)             */
+    DEDISP_ESHAPE = 4, /* strides / lengths inconsistent with the plan                    */
+    DEDISP_ESTATE = 5  /* call not valid for this kind of plan or stream                  */
+} dedisp_status;
+
+typedef enum {
+    DEDISP_F32 = 0, /* float input, float output (fp32 adds)                               */
+    DEDISP_U8 = 1   /* uint8 input (0..255, no offset removed), int32 output, exact       */
+} dedisp_dtype;
+
+/* Kernel choice for dedisp_plan_set_kernel (brute-force plans).  AUTO picks the register-window
+ * kernel when the plan's shift table fits its limits and the direct kernel otherwise. */
+typedef enum {
+    DEDISP_KERNEL_AUTO = 0,
+    DEDISP_KERNEL_NAIVE = 1,  /* one thread per output sample, global loads only (debug)    */
+    DEDISP_KERNEL_DIRECT = 2, /* shared-memory staged, register-blocked DMs x time           */
+    DEDISP_KERNEL_WINDOW = 3  /* + one register window shared by the DM rows of a thread     */
+} dedisp_kernel;
+
+/*
+ * dedisp_plan_create -- build the integer shift table(s) of eq. 1 on the host.
+ *
+ *   nchans      number of frequency channels (> 0)
+ *   f_top_mhz   frequency of channel 0, the highest, in MHz (> 0)
+ *   df_mhz      magnitude of the channel width in MHz (> 0); f_c = f_top - c*df must stay > 0
+ *   t_samp_ms   sampling time in ms (> 0)
+ *   dm_list     HOST, ndm doubles, pc cm^-3, finite and >= 0; copied
+ *   ndm         number of DM trials (> 0)
+ *   nsub        0: brute-force plan.  > 0: two-stage subband plan with nsub subbands of
+ *               nchans/nsub consecutive channels (nchans % nsub == 0)
+ *   nfine       subband plans only: dm_list is ndm/nfine consecutive groups of nfine trials
+ *               (ndm % nfine == 0, dm_list non-decreasing); group k is partially de-dispersed at
+ *               its nominal DM dm_list[k*nfine + nfine/2].  Ignored when nsub == 0.
+ *
+ * shift(c,d) = (int32) floor(x + 0.5), x evaluated in IEEE fp64, every operation rounded on its
+ * own, in this order:  f_c = f_top - (double)c*df;  a_c = 1/(f_c*f_c) - 1/(f_top*f_top);
+ * k_c = 4.15e6*a_c;  x = (k_c*DM_d)/t_samp.
+ * Subband tables: s1(c,k) = shift(c,D_k) - shift(ctop(s),D_k), s2(d,s) = shift(ctop(s),DM_d),
+ * ctop(s) = s*nchans/nsub.
+ *
+ * On success *plan is a new plan.  Errors: DEDISP_EINVAL (any rule above violated, a shift that
+ * does not fit int32), DEDISP_ENOMEM.  *plan is NULL on error.
+ */
+DEDISP_API dedisp_status dedisp_plan_create(dedisp_plan **plan, int nchans, double f_top_mhz, double df_mhz,
+                                 double t_samp_ms, const double *dm_list, int ndm, int nsub,
+                                 int nfine);
+
+/* Releases the plan, its device tables and scratch.  NULL is accepted.  Streams created from the
+ * plan must be destroyed first. */
+DEDISP_API dedisp_status dedisp_plan_destroy(dedisp_plan *plan);
+
+/* Number of extra input samples per channel the caller must supply beyond nsamp_out
+ * ("maxshift"): the maximum of the integer table (brute force) or of s1+s2
+ * (subband).  -1 if plan is NULL. */
+DEDISP_API int64_t dedisp_plan_max_delay(const dedisp_plan *plan);
+
+/* Scalar properties; -1 if plan is NULL. */
+DEDISP_API int dedisp_plan_nchans(const dedisp_plan *plan);
+DEDISP_API int dedisp_plan_ndm(const dedisp_plan *plan);
+DEDISP_API int dedisp_plan_nsub(const dedisp_plan *plan);
+DEDISP_API int dedisp_plan_nfine(const dedisp_plan *plan);
+
+/* Copies the full-band table shift[ndm][nchans] (row d = DM trial d) to HOST memory.
+ * Valid for both kinds of plan (for subband plans it is the table s1/s2 derive from). */
+DEDISP_API dedisp_status dedisp_plan_get_shifts(const dedisp_plan *plan, int32_t *host_out);
+
+/* Subband plans: s1 [ncoarse][nchans], s2 [ndm][nsub], nominal_dm [ncoarse],
+ * maxshift2 [ncoarse] (overlap stage 1 keeps for stage 2); all HOST; any may be
+ * NULL.  DEDISP_ESTATE for brute-force plans. */
+DEDISP_API dedisp_status dedisp_plan_get_subband_shifts(const dedisp_plan *plan, int32_t *s1, int32_t *s2,
+                                             double *nominal_dm, int32_t *maxshift2);
+
+/* Selects the brute-force kernel (default DEDISP_KERNEL_AUTO).  DEDISP_EINVAL for an unknown
+ * value, DEDISP_ESTATE if WINDOW is forced on a plan whose table exceeds its limits. */
+DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel kernel);
+
+/* Which kernel AUTO resolves to for this plan and dtype (a dedisp_kernel value), -1 on error. */
+DEDISP_API int dedisp_plan_resolved_kernel(const dedisp_plan *plan, dedisp_dtype dtype);
+
+/* Bytes of device scratch a subband execute of nsamp_out samples and nbeams beams needs
+ * (the stage-1 intermediate, fp32 or int32); 0 for brute-force plans; -1 on error. */
+DEDISP_API int64_t dedisp_plan_scratch_bytes(const dedisp_plan *plan, int64_t nsamp_out, int nbeams);
+
+/*
+ * dedisp_execute -- de-disperse one resident buffer.
+ *
+ *   in          DEVICE, [nbeams][nchans][in_stride] elements of dtype's input type (float or
+ *               uint8); in_stride >= nsamp_out + max_delay; for DEDISP_F32 the pointer and
+ *               in_stride*4 must be multiples of 16 bytes, for DEDISP_U8 of 16 bytes as well
+ *   out         DEVICE, [nbeams][ndm][out_stride] float (F32) or int32 (U8); out_stride >=
+ *               nsamp_out; pointer 16-byte aligned and out_stride a multiple of 4
+ *   nsamp_out   output samples per DM trial (>= 0; 0 is a no-op)
+ *   cuda_stream a cudaStream_t (NULL = the legacy default stream)
+ *
+ * Brute-force plans: one kernel.  Subband plans: stage 1 into the plan's scratch (grown on
+ * demand, so one execute per plan may be in flight), then stage 2.  Input elements beyond
+ * nsamp_out + max_delay in a row are never read; output elements beyond nsamp_out in a row are
+ * never written.  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ENOMEM, DEDISP_ECUDA.
+ */
+DEDISP_API dedisp_status dedisp_execute(dedisp_plan *plan, const void *in, void *out, dedisp_dtype dtype,
+                             int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
+                             void *cuda_stream);
+
+/*
+ * Host-buffer convenience: same operation with HOST in/out ([nbeams][nchans][nsamp_out+max_delay]
+ * dense input, [nbeams][ndm][nsamp_out] dense output).  Allocates device buffers, copies in,
+ * executes, copies out and synchronises the stream.  This is the "end-to-end" entry bench.py
+ * times; every arithmetic step still runs in the CUDA kernels.
+ */
+DEDISP_API dedisp_status dedisp_execute_host(dedisp_plan *plan, const void *host_in, void *host_out,
+                                  dedisp_dtype dtype, int64_t nsamp_out, int nbeams,
+                                  void *cuda_stream);
+
+/*
+ * Streaming chunk driver.  The stream owns a DEVICE work buffer
+ * [nbeams][nchans][max_delay + chunk] whose first max_delay samples per channel are the tail of
+ * the previous chunks (zeros before the first push).  Push k (k = 0, 1, ...) consumes stream
+ * samples [k*chunk, (k+1)*chunk) and produces outputs for stream times
+ * [k*chunk - max_delay, (k+1)*chunk - max_delay); outputs at negative times are warm-up values.
+ * The concatenation of all pushes equals one dedisp_execute over the whole stream, also when
+ * max_delay > chunk.  Brute-force plans only (DEDISP_ESTATE otherwise).
+ *
+ *   chunk_in    DEVICE, [nbeams][nchans][chunk] dense
+ *   out         DEVICE, [nbeams][ndm][chunk] dense
+ */
+DEDISP_API dedisp_status dedisp_stream_create(dedisp_stream **s, dedisp_plan *plan, dedisp_dtype dtype,
+                                   int64_t chunk, int nbeams);
+DEDISP_API dedisp_status dedisp_stream_push(dedisp_stream *s, const void *chunk_in, void *out,
+                                 void *cuda_stream);
+/* Same with HOST chunk_in/out (pinned or pageable): H2D copy, push, D2H copy, synchronise. */
+DEDISP_API dedisp_status dedisp_stream_push_host(dedisp_stream *s, const void *host_chunk_in, void *host_out,
+                                      void *cuda_stream);
+/* Resets the carry to zeros (asynchronously on cuda_stream). */
+DEDISP_API dedisp_status dedisp_stream_reset(dedisp_stream *s, void *cuda_stream);
+DEDISP_API dedisp_status dedisp_stream_destroy(dedisp_stream *s);
+
+/* Largest chunk (output samples per push) such that work buffer + output fit in mem_bytes of
+ * device memory: the paper's eq. 3,
+ * n_samp = (memory - maxshift*n_chans*in_size) / (n_dms*out_size + n_chans*in_size), per beam.
+ * Returns <= 0 if nothing fits; -1 on bad arguments. */
+DEDISP_API int64_t dedisp_plan_max_chunk(const dedisp_plan *plan, dedisp_dtype dtype, int64_t mem_bytes,
+                              int nbeams);
+
+/* Number of kernels the last execute/push on this plan launched (bench.py's gpu_launches). */
+DEDISP_API int dedisp_plan_last_launches(const dedisp_plan *plan);
+
+/* Static string for a status code. */
+DEDISP_API const char *dedisp_strerror(dedisp_status status);
+
+/* Library version string, e.g. "dedisp-b200 0.1 (sm_100a)". */
+DEDISP_API const char *dedisp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DEDISP_H */

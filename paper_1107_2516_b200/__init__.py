@@ -1,0 +1,10 @@
+"""B200-native incoherent de-dispersion (hot path of Magro et al., arXiv 1107.2516).
+
+The product is the C-ABI library built from ``csrc/`` (``include/dedisp.h``); this package holds
+its build script, a ctypes binding with the same names, and the seeded input generators.
+"""
+from .binding import (Plan, Stream, DedispError, F32, U8, KERNEL_AUTO, KERNEL_NAIVE, KERNEL_DIRECT,
+                      KERNEL_WINDOW, lib, version, EXPORTS, LIB_PATH)
+
+__all__ = ["Plan", "Stream", "DedispError", "F32", "U8", "KERNEL_AUTO", "KERNEL_NAIVE",
+           "KERNEL_DIRECT", "KERNEL_WINDOW", "lib", "version", "EXPORTS", "LIB_PATH"]

@@ -1,0 +1,238 @@
+"""Thin ctypes binding of libdedisp_b200.so (include/dedisp.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every arithmetic step runs in the library's CUDA
+kernels.  There is no fallback: if the shared library is missing or a call fails this raises.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdedisp_b200.so")
+
+OK, EINVAL, ENOMEM, ECUDA, ESHAPE, ESTATE = range(6)
+F32, U8 = 0, 1
+KERNEL_AUTO, KERNEL_NAIVE, KERNEL_DIRECT, KERNEL_WINDOW = range(4)
+
+_c = ctypes
+_vp, _i64, _int, _dbl = _c.c_void_p, _c.c_int64, _c.c_int, _c.c_double
+_SIGS = {
+    "dedisp_plan_create": (_int, [_c.POINTER(_vp), _int, _dbl, _dbl, _dbl, _c.POINTER(_dbl), _int, _int, _int]),
+    "dedisp_plan_destroy": (_int, [_vp]),
+    "dedisp_plan_max_delay": (_i64, [_vp]),
+    "dedisp_plan_nchans": (_int, [_vp]),
+    "dedisp_plan_ndm": (_int, [_vp]),
+    "dedisp_plan_nsub": (_int, [_vp]),
+    "dedisp_plan_nfine": (_int, [_vp]),
+    "dedisp_plan_get_shifts": (_int, [_vp, _vp]),
+    "dedisp_plan_get_subband_shifts": (_int, [_vp, _vp, _vp, _vp, _vp]),
+    "dedisp_plan_set_kernel": (_int, [_vp, _int]),
+    "dedisp_plan_resolved_kernel": (_int, [_vp, _int]),
+    "dedisp_plan_scratch_bytes": (_i64, [_vp, _i64, _int]),
+    "dedisp_execute": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _vp]),
+    "dedisp_execute_host": (_int, [_vp, _vp, _vp, _int, _i64, _int, _vp]),
+    "dedisp_stream_create": (_int, [_c.POINTER(_vp), _vp, _int, _i64, _int]),
+    "dedisp_stream_push": (_int, [_vp, _vp, _vp, _vp]),
+    "dedisp_stream_push_host": (_int, [_vp, _vp, _vp, _vp]),
+    "dedisp_stream_reset": (_int, [_vp, _vp]),
+    "dedisp_stream_destroy": (_int, [_vp]),
+    "dedisp_plan_max_chunk": (_i64, [_vp, _int, _i64, _int]),
+    "dedisp_plan_last_launches": (_int, [_vp]),
+    "dedisp_strerror": (_c.c_char_p, [_int]),
+    "dedisp_version": (_c.c_char_p, []),
+}
+EXPORTS = tuple(_SIGS)
+_lib = None
+
+
+class DedispError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        msg = lib().dedisp_strerror(status).decode()
+        super().__init__("%s: %s (status %d)" % (where, msg, status))
+
+
+def lib():
+    """Loads the C-ABI library; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("%s is missing: run `python -m paper_1107_2516_b200.build` "
+                               "(there is no CPU fallback)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in _SIGS.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def _check(status, where):
+    if status != OK:
+        raise DedispError(status, where)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def _dtype_of(t):
+    import torch
+    if t.dtype == torch.float32:
+        return F32, torch.float32
+    if t.dtype == torch.uint8:
+        return U8, torch.int32
+    raise TypeError("input must be float32 or uint8")
+
+
+class Plan:
+    """dedisp_plan_create(nchans, f_top, df, t_samp, dm_list[, nsub, nfine])."""
+
+    def __init__(self, nchans, f_top_mhz, df_mhz, t_samp_ms, dm_list, nsub=0, nfine=0):
+        dm = np.ascontiguousarray(dm_list, dtype=np.float64)
+        h = _vp()
+        _check(lib().dedisp_plan_create(ctypes.byref(h), int(nchans), float(f_top_mhz), float(df_mhz),
+                                        float(t_samp_ms), dm.ctypes.data_as(_c.POINTER(_dbl)),
+                                        int(dm.size), int(nsub), int(nfine)), "dedisp_plan_create")
+        self._h = h
+        self.nchans, self.ndm, self.nsub, self.nfine = int(nchans), int(dm.size), int(nsub), int(nfine)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _check(lib().dedisp_plan_destroy(self._h), "dedisp_plan_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def max_delay(self):
+        return int(lib().dedisp_plan_max_delay(self._h))
+
+    def shifts(self):
+        out = np.empty((self.ndm, self.nchans), dtype=np.int32)
+        _check(lib().dedisp_plan_get_shifts(self._h, out.ctypes.data), "dedisp_plan_get_shifts")
+        return out
+
+    def subband_shifts(self):
+        nco = self.ndm // self.nfine if self.nfine else 0
+        s1 = np.empty((nco, self.nchans), dtype=np.int32)
+        s2 = np.empty((self.ndm, max(self.nsub, 1)), dtype=np.int32)
+        nom = np.empty(nco, dtype=np.float64)
+        m2 = np.empty(nco, dtype=np.int32)
+        _check(lib().dedisp_plan_get_subband_shifts(self._h, s1.ctypes.data, s2.ctypes.data,
+                                                    nom.ctypes.data, m2.ctypes.data),
+               "dedisp_plan_get_subband_shifts")
+        return s1, s2, nom, m2
+
+    def set_kernel(self, kernel):
+        _check(lib().dedisp_plan_set_kernel(self._h, int(kernel)), "dedisp_plan_set_kernel")
+
+    def resolved_kernel(self, dtype=F32):
+        return int(lib().dedisp_plan_resolved_kernel(self._h, int(dtype)))
+
+    def scratch_bytes(self, nsamp_out, nbeams=1):
+        return int(lib().dedisp_plan_scratch_bytes(self._h, int(nsamp_out), int(nbeams)))
+
+    def max_chunk(self, dtype, mem_bytes, nbeams=1):
+        return int(lib().dedisp_plan_max_chunk(self._h, int(dtype), int(mem_bytes), int(nbeams)))
+
+    @property
+    def last_launches(self):
+        return int(lib().dedisp_plan_last_launches(self._h))
+
+    def execute(self, x, nsamp_out, out=None, stream=None):
+        """x: CUDA tensor [nchans][n_in] or [nbeams][nchans][n_in] (float32 or uint8), last dim
+        contiguous, row stride a multiple of 16 bytes.  Returns out [.. ndm][nsamp_out]."""
+        import torch
+        if not x.is_cuda:
+            raise RuntimeError("dedisp_execute needs a CUDA tensor (there is no CPU fallback)")
+        dt, odt = _dtype_of(x)
+        x3 = x if x.dim() == 3 else x.unsqueeze(0)
+        nb, nch, _ = x3.shape
+        if nch != self.nchans or x3.stride(2) != 1 or (nb > 1 and x3.stride(0) != nch * x3.stride(1)):
+            raise DedispError(ESHAPE, "dedisp_execute")
+        if out is None:
+            ostride = (int(nsamp_out) + 3) // 4 * 4
+            buf = torch.empty((nb, self.ndm, ostride), dtype=odt, device=x.device)
+            out3 = buf[:, :, :int(nsamp_out)]
+        else:
+            out3 = out if out.dim() == 3 else out.unsqueeze(0)
+            if out3.dtype != odt or out3.stride(2) != 1 or out3.shape[1] != self.ndm or \
+                    (nb > 1 and out3.stride(0) != self.ndm * out3.stride(1)):
+                raise DedispError(ESHAPE, "dedisp_execute")
+        _check(lib().dedisp_execute(self._h, x3.data_ptr(), out3.data_ptr(), dt, int(nsamp_out),
+                                    int(x3.stride(1)), int(out3.stride(1)), int(nb), _stream_ptr(stream)),
+               "dedisp_execute")
+        return out3 if x.dim() == 3 else out3[0]
+
+    def execute_host(self, x, nsamp_out, out=None, stream=None):
+        """x: numpy / CPU tensor [nbeams][nchans][nsamp_out+max_delay] dense; returns numpy out."""
+        xa = x.numpy() if hasattr(x, "numpy") else np.asarray(x)
+        xa = xa if xa.ndim == 3 else xa[None]
+        assert xa.flags.c_contiguous and xa.shape[1] == self.nchans
+        assert xa.shape[2] == nsamp_out + self.max_delay
+        dt = F32 if xa.dtype == np.float32 else U8
+        if out is None:
+            out = np.empty((xa.shape[0], self.ndm, nsamp_out), dtype=np.float32 if dt == F32 else np.int32)
+        oa = out.numpy() if hasattr(out, "numpy") else out
+        _check(lib().dedisp_execute_host(self._h, xa.ctypes.data, oa.ctypes.data, dt, int(nsamp_out),
+                                         int(xa.shape[0]), _stream_ptr(stream)), "dedisp_execute_host")
+        return out
+
+
+class Stream:
+    """dedisp_stream_*: streaming chunk driver carrying the max_delay overlap between chunks."""
+
+    def __init__(self, plan, dtype, chunk, nbeams=1):
+        h = _vp()
+        _check(lib().dedisp_stream_create(ctypes.byref(h), plan._h, int(dtype), int(chunk), int(nbeams)),
+               "dedisp_stream_create")
+        self._h, self.plan, self.dtype, self.chunk, self.nbeams = h, plan, int(dtype), int(chunk), int(nbeams)
+
+    def push(self, chunk_in, out=None, stream=None):
+        import torch
+        if not chunk_in.is_cuda or not chunk_in.is_contiguous():
+            raise RuntimeError("dedisp_stream_push needs a contiguous CUDA tensor")
+        want = (self.nbeams, self.plan.nchans, self.chunk)
+        if tuple(chunk_in.shape) != want:
+            raise DedispError(ESHAPE, "dedisp_stream_push")
+        if out is None:
+            out = torch.empty((self.nbeams, self.plan.ndm, self.chunk), device=chunk_in.device,
+                              dtype=torch.float32 if self.dtype == F32 else torch.int32)
+        _check(lib().dedisp_stream_push(self._h, chunk_in.data_ptr(), out.data_ptr(), _stream_ptr(stream)),
+               "dedisp_stream_push")
+        return out
+
+    def push_host(self, chunk_in, out, stream=None):
+        ia = chunk_in.numpy() if hasattr(chunk_in, "numpy") else chunk_in
+        oa = out.numpy() if hasattr(out, "numpy") else out
+        assert ia.flags.c_contiguous and oa.flags.c_contiguous
+        _check(lib().dedisp_stream_push_host(self._h, ia.ctypes.data, oa.ctypes.data, _stream_ptr(stream)),
+               "dedisp_stream_push_host")
+        return out
+
+    def reset(self, stream=None):
+        _check(lib().dedisp_stream_reset(self._h, _stream_ptr(stream)), "dedisp_stream_reset")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _check(lib().dedisp_stream_destroy(self._h), "dedisp_stream_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def version():
+    return lib().dedisp_version().decode()

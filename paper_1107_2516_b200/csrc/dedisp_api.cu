@@ -1,0 +1,586 @@
+// C ABI of libdedisp_b200.so (include/dedisp.h): plans, execute, the streaming chunk driver.
+// Host-side only; the arithmetic lives in shift_table.cpp (tables) and kernels_*.cu (sums).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "dedisp_internal.h"
+
+using namespace dedisp;
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t bytes = 0;
+    cudaError_t ensure(size_t n)
+    {
+        if (n <= bytes)
+            return cudaSuccess;
+        if (p)
+            cudaFree(p);
+        p = nullptr;
+        bytes = 0;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e == cudaSuccess)
+            bytes = n;
+        return e;
+    }
+    void release()
+    {
+        if (p)
+            cudaFree(p);
+        p = nullptr;
+        bytes = 0;
+    }
+};
+
+// max over row tiles [k*tile, (k+1)*tile) and columns of (max - min) of table[row][col]
+int tile_spread(const int32_t* tab, int nrows, int ncols, int64_t row_stride, int tile)
+{
+    int worst = 0;
+    std::vector<int32_t> mn(ncols), mx(ncols);
+    for (int r0 = 0; r0 < nrows; r0 += tile) {
+        const int r1 = r0 + tile < nrows ? r0 + tile : nrows;
+        for (int c = 0; c < ncols; ++c)
+            mn[c] = mx[c] = tab[static_cast<int64_t>(r0) * row_stride + c];
+        for (int r = r0 + 1; r < r1; ++r) {
+            const int32_t* row = tab + static_cast<int64_t>(r) * row_stride;
+            for (int c = 0; c < ncols; ++c) {
+                mn[c] = row[c] < mn[c] ? row[c] : mn[c];
+                mx[c] = row[c] > mx[c] ? row[c] : mx[c];
+            }
+        }
+        for (int c = 0; c < ncols; ++c)
+            worst = mx[c] - mn[c] > worst ? mx[c] - mn[c] : worst;
+    }
+    return worst;
+}
+
+int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+}  // namespace
+
+struct dedisp_plan {
+    int nchans = 0, ndm = 0, nsub = 0, nfine = 0;
+    double f_top = 0, df = 0, t_samp = 0;
+    std::vector<double> dm;
+    std::vector<int32_t> shift;  // [ndm][nchans]
+    int64_t max_delay = 0;       // what the caller must supply (brute: table max; subband: s1+s2)
+    int spread_full[3] = {0, 0, 0};
+    // subband
+    std::vector<int32_t> s1, s2, maxshift2;
+    std::vector<double> nominal;
+    int32_t maxshift2_max = 0;
+    int spread_s1[3] = {0, 0, 0}, spread_s2[3] = {0, 0, 0};
+    // device side (uploaded by the first execute)
+    bool uploaded = false;
+    int device = -1;
+    int32_t *d_shift = nullptr, *d_s1 = nullptr, *d_s2 = nullptr, *d_maxshift2 = nullptr;
+    DevBuf scratch;            // subband intermediate
+    DevBuf host_in, host_out;  // staging for dedisp_execute_host
+    dedisp_kernel kernel = DEDISP_KERNEL_AUTO;
+    int last_launches = 0;
+    int nstreams = 0;
+};
+
+struct dedisp_stream {
+    dedisp_plan* plan = nullptr;
+    dedisp_dtype dtype = DEDISP_F32;
+    int64_t chunk = 0, wstride = 0;
+    int nbeams = 0;
+    DevBuf work[2];
+    int cur = 0;
+    bool zeroed = false;
+    DevBuf host_in, host_out;
+};
+
+namespace {
+
+size_t in_size(dedisp_dtype t) { return t == DEDISP_F32 ? 4 : 1; }
+
+dedisp_status upload(dedisp_plan* p)
+{
+    if (p->uploaded)
+        return DEDISP_OK;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess)
+        return DEDISP_ECUDA;
+    auto up = [](int32_t** d, const std::vector<int32_t>& h) -> cudaError_t {
+        if (h.empty())
+            return cudaSuccess;
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(d), h.size() * sizeof(int32_t));
+        if (e != cudaSuccess)
+            return e;
+        return cudaMemcpy(*d, h.data(), h.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+    };
+    cudaError_t e = cudaSuccess;
+    if (p->nsub == 0) {
+        e = up(&p->d_shift, p->shift);
+    } else {
+        e = up(&p->d_s1, p->s1);
+        if (e == cudaSuccess)
+            e = up(&p->d_s2, p->s2);
+        if (e == cudaSuccess)
+            e = up(&p->d_maxshift2, p->maxshift2);
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA;
+    }
+    p->device = dev;
+    p->uploaded = true;
+    return DEDISP_OK;
+}
+
+int run_problem(dedisp_plan* plan, const Problem& pr, Elem in_t, const int spread[3], void* stream)
+{
+    switch (plan->kernel) {
+    case DEDISP_KERNEL_NAIVE: return launch_naive(pr, in_t, stream, &plan->last_launches);
+    default: return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
+    }
+}
+
+dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedisp_dtype dtype,
+                             int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
+                             void* stream)
+{
+    if (!plan || nbeams <= 0 || nsamp_out < 0 || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    if (nsamp_out == 0) {
+        plan->last_launches = 0;
+        return DEDISP_OK;
+    }
+    if (!in || !out)
+        return DEDISP_EINVAL;
+    const int64_t vec = 16 / static_cast<int64_t>(in_size(dtype));
+    if (in_stride < nsamp_out + plan->max_delay || out_stride < nsamp_out || in_stride % vec != 0 ||
+        out_stride % 4 != 0 || (reinterpret_cast<uintptr_t>(in) & 15) != 0 ||
+        (reinterpret_cast<uintptr_t>(out) & 15) != 0)
+        return DEDISP_ESHAPE;
+    plan->last_launches = 0;
+    dedisp_status st = upload(plan);
+    if (st != DEDISP_OK)
+        return st;
+    const Elem in_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::U8;
+
+    Problem pr;
+    std::memset(&pr, 0, sizeof(pr));
+    pr.nb0 = nbeams;
+    pr.in_len = in_stride;
+    int rc = 0;
+    if (plan->nsub == 0) {
+        pr.in = in;
+        pr.out = out;
+        pr.shift = plan->d_shift;
+        pr.in_chan_stride = in_stride;
+        pr.in_b0_stride = in_stride * plan->nchans;
+        pr.out_dm_stride = out_stride;
+        pr.out_b0_stride = out_stride * plan->ndm;
+        pr.shift_dm_stride = plan->nchans;
+        pr.n_out = pr.n_base = nsamp_out;
+        pr.nchans = plan->nchans;
+        pr.ndm = plan->ndm;
+        pr.nb1 = 1;
+        rc = run_problem(plan, pr, in_t, plan->spread_full, stream);
+        return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
+    }
+
+    // two-stage subband: stage 1 into scratch, stage 2 from scratch
+    const int ncoarse = plan->ndm / plan->nfine, cps = plan->nchans / plan->nsub;
+    const int64_t n1 = round_up(nsamp_out + plan->maxshift2_max, 16);
+    const size_t need = static_cast<size_t>(nbeams) * ncoarse * plan->nsub * n1 * 4;
+    if (plan->scratch.ensure(need) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    // stage 1: b1 = subband s, rows = coarse groups k, channels = the cps channels of s
+    pr.in = in;
+    pr.out = plan->scratch.p;
+    pr.shift = plan->d_s1;
+    pr.row_extra = plan->d_maxshift2;
+    pr.in_chan_stride = in_stride;
+    pr.in_b0_stride = in_stride * plan->nchans;
+    pr.in_b1_stride = in_stride * cps;
+    pr.out_dm_stride = n1 * plan->nsub;
+    pr.out_b0_stride = n1 * plan->nsub * ncoarse;
+    pr.out_b1_stride = n1;
+    pr.shift_dm_stride = plan->nchans;
+    pr.shift_b1_stride = cps;
+    pr.n_base = nsamp_out;
+    pr.n_out = nsamp_out + plan->maxshift2_max;
+    pr.nchans = cps;
+    pr.ndm = ncoarse;
+    pr.nb1 = plan->nsub;
+    rc = run_problem(plan, pr, in_t, plan->spread_s1, stream);
+    if (rc != 0)
+        return DEDISP_ECUDA;
+    // stage 2: b1 = coarse group k, rows = its nfine trials, channels = the nsub partial series
+    Problem p2;
+    std::memset(&p2, 0, sizeof(p2));
+    p2.in = plan->scratch.p;
+    p2.out = out;
+    p2.shift = plan->d_s2;
+    p2.in_chan_stride = n1;
+    p2.in_b0_stride = n1 * plan->nsub * ncoarse;
+    p2.in_b1_stride = n1 * plan->nsub;
+    p2.in_len = n1;
+    p2.out_dm_stride = out_stride;
+    p2.out_b0_stride = out_stride * plan->ndm;
+    p2.out_b1_stride = out_stride * plan->nfine;
+    p2.shift_dm_stride = plan->nsub;
+    p2.shift_b1_stride = static_cast<int64_t>(plan->nsub) * plan->nfine;
+    p2.n_out = p2.n_base = nsamp_out;
+    p2.nchans = plan->nsub;
+    p2.ndm = plan->nfine;
+    p2.nb0 = nbeams;
+    p2.nb1 = ncoarse;
+    rc = run_problem(plan, p2, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, plan->spread_s2, stream);
+    return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+}  // namespace
+
+extern "C" {
+
+dedisp_status dedisp_plan_create(dedisp_plan** plan, int nchans, double f_top_mhz, double df_mhz,
+                                 double t_samp_ms, const double* dm_list, int ndm, int nsub, int nfine)
+{
+    if (!plan)
+        return DEDISP_EINVAL;
+    *plan = nullptr;
+    if (nchans <= 0 || ndm <= 0 || !dm_list || !(f_top_mhz > 0.0) || !(df_mhz > 0.0) ||
+        !(t_samp_ms > 0.0) || !std::isfinite(f_top_mhz) || !std::isfinite(df_mhz) ||
+        !std::isfinite(t_samp_ms) || nsub < 0)
+        return DEDISP_EINVAL;
+    if (!(f_top_mhz - static_cast<double>(nchans - 1) * df_mhz > 0.0))
+        return DEDISP_EINVAL;
+    for (int d = 0; d < ndm; ++d)
+        if (!(dm_list[d] >= 0.0) || !std::isfinite(dm_list[d]))
+            return DEDISP_EINVAL;
+    if (nsub > 0) {
+        if (nfine <= 0 || nchans % nsub != 0 || ndm % nfine != 0)
+            return DEDISP_EINVAL;
+        for (int d = 1; d < ndm; ++d)
+            if (dm_list[d] < dm_list[d - 1])
+                return DEDISP_EINVAL;
+    }
+    dedisp_plan* p = new (std::nothrow) dedisp_plan;
+    if (!p)
+        return DEDISP_ENOMEM;
+    try {
+        p->nchans = nchans;
+        p->ndm = ndm;
+        p->nsub = nsub;
+        p->nfine = nsub > 0 ? nfine : 0;
+        p->f_top = f_top_mhz;
+        p->df = df_mhz;
+        p->t_samp = t_samp_ms;
+        p->dm.assign(dm_list, dm_list + ndm);
+        if (!build_shift_table(nchans, f_top_mhz, df_mhz, t_samp_ms, dm_list, ndm, p->shift,
+                               p->max_delay)) {
+            delete p;
+            return DEDISP_EINVAL;
+        }
+        const int tiles[3] = {32, 16, 8};
+        if (nsub == 0) {
+            for (int k = 0; k < 3; ++k)
+                p->spread_full[k] = tile_spread(p->shift.data(), ndm, nchans, nchans, tiles[k]);
+        } else {
+            build_subband_tables(p->shift, nchans, ndm, nsub, nfine, dm_list, p->s1, p->s2, p->nominal,
+                                 p->maxshift2, p->max_delay);
+            const int ncoarse = ndm / nfine;
+            for (int k = 0; k < ncoarse; ++k)
+                p->maxshift2_max = p->maxshift2[k] > p->maxshift2_max ? p->maxshift2[k] : p->maxshift2_max;
+            for (int k = 0; k < 3; ++k) {
+                p->spread_s1[k] = tile_spread(p->s1.data(), ncoarse, nchans, nchans, tiles[k]);
+                int w = 0;
+                for (int g = 0; g < ncoarse; ++g) {
+                    const int v = tile_spread(p->s2.data() + static_cast<size_t>(g) * nfine * nsub, nfine,
+                                              nsub, nsub, tiles[k]);
+                    w = v > w ? v : w;
+                }
+                p->spread_s2[k] = w;
+            }
+        }
+    } catch (const std::bad_alloc&) {
+        delete p;
+        return DEDISP_ENOMEM;
+    }
+    *plan = p;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_plan_destroy(dedisp_plan* p)
+{
+    if (!p)
+        return DEDISP_OK;
+    if (p->nstreams != 0)
+        return DEDISP_ESTATE;
+    if (p->uploaded) {
+        cudaFree(p->d_shift);
+        cudaFree(p->d_s1);
+        cudaFree(p->d_s2);
+        cudaFree(p->d_maxshift2);
+    }
+    p->scratch.release();
+    p->host_in.release();
+    p->host_out.release();
+    delete p;
+    return DEDISP_OK;
+}
+
+int64_t dedisp_plan_max_delay(const dedisp_plan* p) { return p ? p->max_delay : -1; }
+int dedisp_plan_nchans(const dedisp_plan* p) { return p ? p->nchans : -1; }
+int dedisp_plan_ndm(const dedisp_plan* p) { return p ? p->ndm : -1; }
+int dedisp_plan_nsub(const dedisp_plan* p) { return p ? p->nsub : -1; }
+int dedisp_plan_nfine(const dedisp_plan* p) { return p ? p->nfine : -1; }
+int dedisp_plan_last_launches(const dedisp_plan* p) { return p ? p->last_launches : -1; }
+
+dedisp_status dedisp_plan_get_shifts(const dedisp_plan* p, int32_t* host_out)
+{
+    if (!p || !host_out)
+        return DEDISP_EINVAL;
+    std::memcpy(host_out, p->shift.data(), p->shift.size() * sizeof(int32_t));
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_plan_get_subband_shifts(const dedisp_plan* p, int32_t* s1, int32_t* s2,
+                                             double* nominal_dm, int32_t* maxshift2)
+{
+    if (!p)
+        return DEDISP_EINVAL;
+    if (p->nsub == 0)
+        return DEDISP_ESTATE;
+    if (s1)
+        std::memcpy(s1, p->s1.data(), p->s1.size() * sizeof(int32_t));
+    if (s2)
+        std::memcpy(s2, p->s2.data(), p->s2.size() * sizeof(int32_t));
+    if (nominal_dm)
+        std::memcpy(nominal_dm, p->nominal.data(), p->nominal.size() * sizeof(double));
+    if (maxshift2)
+        std::memcpy(maxshift2, p->maxshift2.data(), p->maxshift2.size() * sizeof(int32_t));
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_plan_set_kernel(dedisp_plan* p, dedisp_kernel k)
+{
+    if (!p || k < DEDISP_KERNEL_AUTO || k > DEDISP_KERNEL_WINDOW)
+        return DEDISP_EINVAL;
+    if (k == DEDISP_KERNEL_WINDOW)
+        return DEDISP_ESTATE;  // not available for this plan
+    p->kernel = k;
+    return DEDISP_OK;
+}
+
+int dedisp_plan_resolved_kernel(const dedisp_plan* p, dedisp_dtype dtype)
+{
+    if (!p || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return -1;
+    return p->kernel == DEDISP_KERNEL_AUTO ? DEDISP_KERNEL_DIRECT : p->kernel;
+}
+
+int64_t dedisp_plan_scratch_bytes(const dedisp_plan* p, int64_t nsamp_out, int nbeams)
+{
+    if (!p || nsamp_out < 0 || nbeams <= 0)
+        return -1;
+    if (p->nsub == 0)
+        return 0;
+    const int64_t n1 = round_up(nsamp_out + p->maxshift2_max, 16);
+    return static_cast<int64_t>(nbeams) * (p->ndm / p->nfine) * p->nsub * n1 * 4;
+}
+
+dedisp_status dedisp_execute(dedisp_plan* plan, const void* in, void* out, dedisp_dtype dtype,
+                             int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
+                             void* cuda_stream)
+{
+    return execute_device(plan, in, out, dtype, nsamp_out, in_stride, out_stride, nbeams, cuda_stream);
+}
+
+dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* host_out,
+                                  dedisp_dtype dtype, int64_t nsamp_out, int nbeams, void* cuda_stream)
+{
+    if (!plan || !host_in || !host_out || nbeams <= 0 || nsamp_out < 0 ||
+        (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    if (nsamp_out == 0)
+        return DEDISP_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t es = in_size(dtype);
+    const int64_t n_in = nsamp_out + plan->max_delay;
+    const int64_t in_stride = round_up(n_in, 16), out_stride = round_up(nsamp_out, 4);
+    const size_t rows_in = static_cast<size_t>(nbeams) * plan->nchans;
+    const size_t rows_out = static_cast<size_t>(nbeams) * plan->ndm;
+    if (plan->host_in.ensure(rows_in * in_stride * es) != cudaSuccess ||
+        plan->host_out.ensure(rows_out * out_stride * 4) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    if (cudaMemcpy2DAsync(plan->host_in.p, in_stride * es, host_in, n_in * es, n_in * es, rows_in,
+                          cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return DEDISP_ECUDA;
+    dedisp_status s = execute_device(plan, plan->host_in.p, plan->host_out.p, dtype, nsamp_out,
+                                     in_stride, out_stride, nbeams, cuda_stream);
+    if (s != DEDISP_OK)
+        return s;
+    if (cudaMemcpy2DAsync(host_out, nsamp_out * 4, plan->host_out.p, out_stride * 4, nsamp_out * 4,
+                          rows_out, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return DEDISP_ECUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+// ---- streaming chunk driver -------------------------------------------------------------------
+
+dedisp_status dedisp_stream_create(dedisp_stream** s, dedisp_plan* plan, dedisp_dtype dtype,
+                                   int64_t chunk, int nbeams)
+{
+    if (!s)
+        return DEDISP_EINVAL;
+    *s = nullptr;
+    if (!plan || chunk <= 0 || nbeams <= 0 || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    if (plan->nsub != 0)
+        return DEDISP_ESTATE;
+    dedisp_stream* q = new (std::nothrow) dedisp_stream;
+    if (!q)
+        return DEDISP_ENOMEM;
+    q->plan = plan;
+    q->dtype = dtype;
+    q->chunk = chunk;
+    q->nbeams = nbeams;
+    q->wstride = round_up(plan->max_delay + chunk, 16);
+    const size_t bytes = static_cast<size_t>(nbeams) * plan->nchans * q->wstride * in_size(dtype);
+    for (int i = 0; i < 2; ++i)
+        if (q->work[i].ensure(bytes) != cudaSuccess) {
+            cudaError_t e = cudaGetLastError();
+            q->work[0].release();
+            q->work[1].release();
+            delete q;
+            return e == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA;
+        }
+    ++plan->nstreams;
+    *s = q;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_stream_reset(dedisp_stream* s, void* cuda_stream)
+{
+    if (!s)
+        return DEDISP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    for (int i = 0; i < 2; ++i)
+        if (cudaMemsetAsync(s->work[i].p, 0, s->work[i].bytes, st) != cudaSuccess)
+            return DEDISP_ECUDA;
+    s->cur = 0;
+    s->zeroed = true;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_stream_push(dedisp_stream* s, const void* chunk_in, void* out, void* cuda_stream)
+{
+    if (!s || !chunk_in || !out)
+        return DEDISP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    if (!s->zeroed) {
+        dedisp_status r = dedisp_stream_reset(s, cuda_stream);
+        if (r != DEDISP_OK)
+            return r;
+    }
+    dedisp_plan* p = s->plan;
+    const size_t es = in_size(s->dtype);
+    const size_t rows = static_cast<size_t>(s->nbeams) * p->nchans;
+    const int64_t M = p->max_delay, C = s->chunk;
+    unsigned char* cur = static_cast<unsigned char*>(s->work[s->cur].p);
+    unsigned char* nxt = static_cast<unsigned char*>(s->work[s->cur ^ 1].p);
+    // 1. the new chunk goes behind the carried max_delay samples of every channel
+    if (cudaMemcpy2DAsync(cur + M * es, s->wstride * es, chunk_in, C * es, C * es, rows,
+                          cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return DEDISP_ECUDA;
+    // 2. de-disperse the work buffer: outputs for stream times [kC - M, (k+1)C - M)
+    dedisp_status r = execute_device(p, cur, out, s->dtype, C, s->wstride, C, s->nbeams, cuda_stream);
+    if (r != DEDISP_OK)
+        return r;
+    // 3. the last max_delay samples become the head of the other buffer (no overlapping copy,
+    //    valid for max_delay > chunk as well)
+    if (M > 0 && cudaMemcpy2DAsync(nxt, s->wstride * es, cur + C * es, s->wstride * es, M * es, rows,
+                                   cudaMemcpyDeviceToDevice, st) != cudaSuccess)
+        return DEDISP_ECUDA;
+    s->cur ^= 1;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_stream_push_host(dedisp_stream* s, const void* host_chunk_in, void* host_out,
+                                      void* cuda_stream)
+{
+    if (!s || !host_chunk_in || !host_out)
+        return DEDISP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    dedisp_plan* p = s->plan;
+    const size_t es = in_size(s->dtype);
+    const size_t nin = static_cast<size_t>(s->nbeams) * p->nchans * s->chunk * es;
+    const size_t nout = static_cast<size_t>(s->nbeams) * p->ndm * s->chunk * 4;
+    if (s->chunk % 4 != 0)
+        return DEDISP_ESHAPE;
+    if (s->host_in.ensure(nin) != cudaSuccess || s->host_out.ensure(nout) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    if (cudaMemcpyAsync(s->host_in.p, host_chunk_in, nin, cudaMemcpyHostToDevice, st) != cudaSuccess)
+        return DEDISP_ECUDA;
+    dedisp_status r = dedisp_stream_push(s, s->host_in.p, s->host_out.p, cuda_stream);
+    if (r != DEDISP_OK)
+        return r;
+    if (cudaMemcpyAsync(host_out, s->host_out.p, nout, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        return DEDISP_ECUDA;
+    return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+dedisp_status dedisp_stream_destroy(dedisp_stream* s)
+{
+    if (!s)
+        return DEDISP_OK;
+    for (int i = 0; i < 2; ++i)
+        s->work[i].release();
+    s->host_in.release();
+    s->host_out.release();
+    if (s->plan)
+        --s->plan->nstreams;
+    delete s;
+    return DEDISP_OK;
+}
+
+int64_t dedisp_plan_max_chunk(const dedisp_plan* p, dedisp_dtype dtype, int64_t mem_bytes, int nbeams)
+{
+    if (!p || mem_bytes <= 0 || nbeams <= 0 || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return -1;
+    // eq. 3 with element sizes and the driver's two work buffers:
+    //   mem >= nbeams * (2 * nchans * (M + n) * in_size + ndm * n * out_size)
+    const double es = static_cast<double>(in_size(dtype));
+    const double per_beam = static_cast<double>(mem_bytes) / nbeams;
+    const double fixed = 2.0 * p->nchans * static_cast<double>(p->max_delay + 16) * es;
+    const double per_samp = 2.0 * p->nchans * es + 4.0 * p->ndm;
+    const double n = (per_beam - fixed) / per_samp;
+    if (!(n >= 1.0))
+        return 0;
+    return static_cast<int64_t>(n) / 16 * 16;
+}
+
+const char* dedisp_strerror(dedisp_status s)
+{
+    switch (s) {
+    case DEDISP_OK: return "ok";
+    case DEDISP_EINVAL: return "invalid argument";
+    case DEDISP_ENOMEM: return "out of memory";
+    case DEDISP_ECUDA: return "CUDA error";
+    case DEDISP_ESHAPE: return "shape, stride or alignment does not match the plan";
+    case DEDISP_ESTATE: return "call not valid for this plan or stream";
+    }
+    return "unknown status";
+}
+
+const char* dedisp_version(void) { return "dedisp-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

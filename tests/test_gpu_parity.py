@@ -1,0 +1,233 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Bars (BASELINE.json north_star): shift tables and uint8->int32 bit-exact;
+fp32 within |gpu - oracle| <= 1e-5 * sum_c |in[c][t+shift]| per output sample."""
+import numpy as np
+import pytest
+
+import paper_1107_2516_b200 as dd
+from paper_1107_2516_b200 import synth, build as ddbuild
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+KERNELS = {"naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT, "auto": dd.KERNEL_AUTO}
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    ddbuild.build()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+
+
+def to_dev(x, pad_to=16):
+    """Host [.., n] -> CUDA tensor whose row stride is a multiple of 16 elements."""
+    n = x.shape[-1]
+    stride = (n + pad_to - 1) // pad_to * pad_to
+    t = torch.zeros(x.shape[:-1] + (stride,), dtype=torch.from_numpy(x[..., :1].copy()).dtype, device="cuda")
+    t[..., :n] = torch.from_numpy(x).cuda()
+    return t[..., :n] if stride == n else t[..., :n]
+
+
+def check_f32(got, ref, sumabs):
+    err = np.abs(got.astype(np.float64) - ref)
+    bound = 1e-5 * sumabs
+    bad = err > bound
+    assert not bad.any(), "fp32 parity: %d outputs beyond 1e-5*sum|in| (worst ratio %.3g)" % (
+        bad.sum(), (err / np.maximum(bound, 1e-300)).max())
+
+
+def small_cfg(dtype="f32", nchans=96, ndm=70, n_out=3000 + 17, step=0.35, seed=21, **kw):
+    return synth.Config("small", nchans, 150.0, 0.1, 0.2, n_out, ndm, step, dtype=dtype, seed=seed,
+                        npulses=3, pulse_width_ms=(0.5, 3.0), pulse_amp=(0.5, 2.0), **kw)
+
+
+def make_case(oracle, cf, n_out=None, beams=1):
+    n_out = n_out or cf.n_out
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    n_in = n_out + int(tab.max())
+    xs = []
+    for b in range(beams):
+        pulses = synth.draw_pulses(cf, n_out, beam=b)
+        xs.append(synth.make_input(cf, n_in, pulses, {p[0]: tab[p[0]] for p in pulses}, beam=b))
+    return tab, np.stack(xs)
+
+
+@pytest.mark.parametrize("kernel", ["naive", "direct", "auto"])
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_brute_small_ragged(oracle, kernel, dtype):
+    cf = small_cfg(dtype)
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    assert (plan.shifts() == tab).all()
+    plan.set_kernel(KERNELS[kernel])
+    got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+    assert plan.last_launches >= 1
+    for b in range(2):
+        if dtype == "u8":
+            assert (got[b] == oracle.brute_u8(x[b], tab, cf.n_out)).all()
+        else:
+            ref, sa = oracle.brute_f32(x[b], tab, cf.n_out)
+            check_f32(got[b], ref, sa)
+
+
+@pytest.mark.parametrize("kernel", ["direct", "auto"])
+def test_cfg1_full(oracle, kernel):
+    cf = synth.configs()[1]
+    tab, x = make_case(oracle, cf)
+    plan = dd.Plan(**cf.plan_args())
+    plan.set_kernel(KERNELS[kernel])
+    got = plan.execute(to_dev(x[0]), cf.n_out).cpu().numpy()
+    ref, sa = oracle.brute_f32(x[0], tab, cf.n_out)
+    check_f32(got, ref, sa)
+    # P7 on the GPU result: the injected pulse is recovered at trial 30
+    w = cf.fixed_pulses[0][2]
+    box = np.cumsum(np.pad(got.astype(np.float64), ((0, 0), (1, 0))), axis=1)
+    assert np.unravel_index(np.argmax(box[:, w:] - box[:, :-w]), (cf.ndm, cf.n_out - w + 1))[0] == 30
+
+
+@pytest.mark.parametrize("k,ndm,n_out", [(2, 256, 4096 + 40), (3, 320, 8192 + 8), (5, 192, 4096)])
+def test_scaled_configs(oracle, k, ndm, n_out):
+    """cfg 2/3/5 geometry (band, t_samp, DM step) on a DM/time subset the oracle finishes quickly;
+    the DM subset is the TOP of the range, where the shifts and their spread are largest."""
+    base = synth.configs()[k]
+    cf = synth.scaled(base, n_out=n_out)
+    full = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    rows = np.r_[0:ndm // 2, cf.ndm - ndm // 2:cf.ndm]
+    dm = cf.dm_list[rows]
+    tab = full[rows]
+    n_in = n_out + int(tab.max())
+    pulses = [(ndm - 5, 100, 20, 1.0), (3, n_out // 2, 8, 2.0)]
+    x = synth.make_input(cf, n_in, pulses, {p[0]: tab[p[0]] for p in pulses})
+    plan = dd.Plan(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, dm)
+    assert (plan.shifts() == tab).all()
+    got = plan.execute(to_dev(x), n_out).cpu().numpy()
+    if cf.dtype == "u8":
+        assert (got == oracle.brute_u8(x, tab, n_out)).all()
+    else:
+        ref, sa = oracle.brute_f32(x, tab, n_out)
+        check_f32(got, ref, sa)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_subband_small(oracle, dtype):
+    cf = small_cfg(dtype, nchans=128, ndm=96, n_out=2048 + 33, step=0.25, nsub=8, nfine=12)
+    tab = oracle.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list,
+                                cf.nsub, cf.nfine)
+    full = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    n_in = cf.n_out + int(full.max())
+    pulses = [(18, 500, 30, 1.5)]
+    x = synth.make_input(cf, n_in, pulses, {18: full[18]})
+    plan = dd.Plan(**cf.plan_args())
+    assert plan.max_delay == tab.max_delay
+    got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+    assert plan.last_launches == 2
+    ref, sa = oracle.subband(x, tab, cf.n_out)
+    if dtype == "u8":
+        assert (got == ref).all()
+        # P8(i): nominal rows equal brute force exactly
+        rows = [k * cf.nfine + cf.nfine // 2 for k in range(tab.ncoarse)]
+        assert (got[rows] == oracle.brute_u8(x, full, cf.n_out)[rows]).all()
+    else:
+        check_f32(got, ref, sa)
+
+
+def test_cfg4_geometry_subband_scaled(oracle):
+    """cfg-4 band and DM grid, 512 of the 4096 channels' subbands kept whole: 4 subbands of 128."""
+    base = synth.configs()[4]
+    cf = synth.scaled(base, nchans=512, nsub=4, n_out=4096 + 12, ndm=256)
+    tab = oracle.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list, 4, 32)
+    full = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    x = synth.make_input(cf, cf.n_out + int(full.max()))
+    plan = dd.Plan(**cf.plan_args())
+    got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+    ref, sa = oracle.subband(x, tab, cf.n_out)
+    check_f32(got, ref, sa)
+
+
+@pytest.mark.parametrize("chunk_rel", ["larger", "smaller"])
+@pytest.mark.parametrize("dtype", ["u8", "f32"])
+def test_streaming_equals_one_shot(oracle, dtype, chunk_rel):
+    cf = small_cfg(dtype, nchans=64, ndm=40, n_out=0, step=0.3)
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    M = int(tab.max())
+    C = (M + 200) // 4 * 4 if chunk_rel == "larger" else max(16, (M // 3) // 4 * 4)
+    npush, beams = 5, 2
+    total = npush * C
+    xs = np.stack([synth.make_input(cf, total, [(7, M + 10, 12, 2.0)], {7: tab[7]}, beam=b)
+                   for b in range(beams)])
+    plan = dd.Plan(**cf.plan_args())
+    st = dd.Stream(plan, dd.U8 if dtype == "u8" else dd.F32, C, beams)
+    outs = []
+    for k in range(npush):
+        outs.append(st.push(torch.from_numpy(np.ascontiguousarray(xs[:, :, k * C:(k + 1) * C])).cuda())
+                    .cpu().numpy())
+    got = np.concatenate(outs, axis=2)[:, :, M:]          # drop the warm-up outputs (reading R9)
+    n = total - M
+    for b in range(beams):
+        if dtype == "u8":
+            assert (got[b] == oracle.brute_u8(xs[b], tab, n)).all()
+        else:
+            ref, sa = oracle.brute_f32(xs[b], tab, n)
+            check_f32(got[b], ref, sa)
+    # warm-up outputs of push 0 see zeros before the stream start
+    st.reset()
+    first = st.push(torch.from_numpy(np.ascontiguousarray(xs[:, :, :C])).cuda()).cpu().numpy()
+    assert (first == outs[0]).all()
+    st.close()
+    plan.close()
+
+
+def test_edge_cases(oracle):
+    # one channel, one DM, one sample; DM 0 only; nsamp_out = 0
+    p = dd.Plan(1, 100.0, 1.0, 1.0, [0.0])
+    x = torch.arange(16, dtype=torch.float32, device="cuda").reshape(1, 16)
+    assert p.execute(x, 1).cpu().tolist() == [[0.0]]
+    assert p.execute(x, 16).cpu().tolist() == [list(map(float, range(16)))]
+    assert p.execute(x, 0).shape == (1, 0) and p.last_launches == 0
+    # input too short for nsamp_out + max_delay, misaligned stride
+    cf = small_cfg()
+    plan = dd.Plan(**cf.plan_args())
+    M = plan.max_delay
+    x = torch.zeros((cf.nchans, (1024 + M + 31) // 16 * 16), dtype=torch.float32, device="cuda")
+    with pytest.raises(dd.DedispError) as e:
+        plan.execute(x, x.shape[1] - M + 1)            # needs one more input sample than there is
+    assert e.value.status == dd.binding.ESHAPE
+    with pytest.raises(dd.DedispError) as e:
+        plan.execute(x[:, 1:], 512)                    # base pointer not 16-byte aligned
+    assert e.value.status == dd.binding.ESHAPE
+    with pytest.raises(RuntimeError):
+        plan.execute(x.cpu(), 16)
+    # constant input (the paper's perf-test buffers): every output = nchans * v
+    x.fill_(0.375)
+    assert (plan.execute(x, 1024).cpu().numpy() == cf.nchans * 0.375).all()
+
+
+def test_execute_host_roundtrip(oracle):
+    cf = small_cfg("u8", n_out=1500)
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    got = plan.execute_host(x, cf.n_out)
+    for b in range(2):
+        assert (got[b] == oracle.brute_u8(x[b], tab, cf.n_out)).all()
+
+
+def test_cfg3_full_size_sampled(oracle):
+    """BASELINE cfg 3 at full size in bench.py's launch configuration; 300 outputs sampled over the
+    whole (DM, time) plane are recomputed one by one by the oracle's definition."""
+    cf = synth.configs()[3]
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    n_in = cf.n_out + int(tab.max())
+    pulses = synth.draw_pulses(cf, cf.n_out)
+    x = synth.make_input(cf, n_in, pulses, {p[0]: tab[p[0]] for p in pulses})
+    plan = dd.Plan(**cf.plan_args())
+    out = plan.execute(to_dev(x), cf.n_out)
+    rng = np.random.default_rng(3)
+    d = np.r_[rng.integers(0, cf.ndm, 280), [0, 0, cf.ndm - 1, cf.ndm - 1] * 5]
+    t = np.r_[rng.integers(0, cf.n_out, 280), [0, cf.n_out - 1] * 10]
+    ref, sa = oracle.brute_samples(x, tab, d, t)
+    got = out[torch.from_numpy(d).cuda(), torch.from_numpy(t).cuda()].cpu().numpy()
+    check_f32(got, ref, sa)
+    # P3-style invariant at full size: DM 0 row is the plain channel sum
+    row0 = out[0].cpu().numpy().astype(np.float64)
+    s0 = x[:, :cf.n_out].sum(axis=0, dtype=np.float64)
+    assert np.abs(row0 - s0).max() <= 1e-5 * np.abs(x[:, :cf.n_out]).sum(axis=0, dtype=np.float64).max()
