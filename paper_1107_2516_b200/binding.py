@@ -29,6 +29,7 @@ _SIGS = {
     "dedisp_plan_get_subband_shifts": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "dedisp_plan_set_kernel": (_int, [_vp, _int]),
     "dedisp_plan_resolved_kernel": (_int, [_vp, _int]),
+    "dedisp_plan_window_info": (_int, [_vp, _vp]),
     "dedisp_plan_scratch_bytes": (_i64, [_vp, _i64, _int]),
     "dedisp_execute": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _vp]),
     "dedisp_execute_host": (_int, [_vp, _vp, _vp, _int, _i64, _int, _vp]),
@@ -137,6 +138,13 @@ class Plan:
 
     def resolved_kernel(self, dtype=F32):
         return int(lib().dedisp_plan_resolved_kernel(self._h, int(dtype)))
+
+    def window_info(self):
+        """dedisp_plan_window_info as a dict (geometry of the register-window kernel)."""
+        a = np.zeros(8, dtype=np.int64)
+        _check(lib().dedisp_plan_window_info(self._h, a.ctypes.data), "dedisp_plan_window_info")
+        keys = ("ok", "H", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "maxbase")
+        return dict(zip(keys, (int(v) for v in a)))
 
     def scratch_bytes(self, nsamp_out, nbeams=1):
         return int(lib().dedisp_plan_scratch_bytes(self._h, int(nsamp_out), int(nbeams)))

@@ -85,6 +85,11 @@ struct dedisp_plan {
     dedisp_kernel kernel = DEDISP_KERNEL_AUTO;
     int last_launches = 0;
     int nstreams = 0;
+    // register-window kernel (brute-force plans): host plan, device tables, pair scratch
+    WindowPlan win;
+    bool win_fits = false;
+    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr;
+    DevBuf pairs;
 };
 
 struct dedisp_stream {
@@ -120,6 +125,11 @@ dedisp_status upload(dedisp_plan* p)
     cudaError_t e = cudaSuccess;
     if (p->nsub == 0) {
         e = up(&p->d_shift, p->shift);
+        if (e == cudaSuccess && p->win.ok) {
+            e = up(&p->d_win_meta, p->win.meta);
+            if (e == cudaSuccess)
+                e = up(&p->d_win_kfinal, p->win.kfinal);
+        }
     } else {
         e = up(&p->d_s1, p->s1);
         if (e == cudaSuccess)
@@ -134,6 +144,47 @@ dedisp_status upload(dedisp_plan* p)
     p->device = dev;
     p->uploaded = true;
     return DEDISP_OK;
+}
+
+bool use_window(const dedisp_plan* p, dedisp_dtype dtype)
+{
+    if (p->nsub != 0 || !p->win.ok || !p->win_fits)
+        return false;
+    // uint8 sums are carried in fp32, exact while nchans * 255 < 2^24
+    if (dtype == DEDISP_U8 && static_cast<int64_t>(p->nchans) * 255 >= (1 << 24))
+        return false;
+    return p->kernel == DEDISP_KERNEL_AUTO || p->kernel == DEDISP_KERNEL_WINDOW;
+}
+
+// brute force through the register-window kernel: pairify into the plan's scratch, then add
+dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t, int64_t nsamp_out,
+                         int64_t in_stride, int64_t out_stride, int nbeams, void* stream)
+{
+    WindowArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.pair_stride = window_pair_stride(plan->win, nsamp_out);
+    const size_t need = static_cast<size_t>(nbeams) * plan->nchans * a.pair_stride * 8;
+    if (plan->pairs.ensure(need) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    a.in = in;
+    a.out = out;
+    a.pairs = plan->pairs.p;
+    a.meta = plan->d_win_meta;
+    a.kfinal = plan->d_win_kfinal;
+    a.in_stride = in_stride;
+    a.out_stride = out_stride;
+    a.in_len = nsamp_out + plan->max_delay;
+    a.n_out = nsamp_out;
+    a.nchans = plan->nchans;
+    a.ndm = plan->ndm;
+    a.nbeams = nbeams;
+    a.H = plan->win.H;
+    a.lmax = plan->win.lmax;
+    a.ntile_dm = plan->win.ntile_dm;
+    a.ntile_t = static_cast<int>((nsamp_out + 2 * plan->win.H - 1) / (2 * plan->win.H));
+    return launch_window(a, in_t, stream, &plan->last_launches) == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
 int run_problem(dedisp_plan* plan, const Problem& pr, Elem in_t, const int spread[3], void* stream)
@@ -172,6 +223,8 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     pr.nb0 = nbeams;
     pr.in_len = in_stride;
     int rc = 0;
+    if (use_window(plan, dtype))
+        return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream);
     if (plan->nsub == 0) {
         pr.in = in;
         pr.out = out;
@@ -289,6 +342,8 @@ dedisp_status dedisp_plan_create(dedisp_plan** plan, int nchans, double f_top_mh
         if (nsub == 0) {
             for (int k = 0; k < 3; ++k)
                 p->spread_full[k] = tile_spread(p->shift.data(), ndm, nchans, nchans, tiles[k]);
+            build_window_plan(p->shift.data(), ndm, nchans, p->win);
+            p->win_fits = p->win.ok && window_fits_smem(p->win.lmax);
         } else {
             build_subband_tables(p->shift, nchans, ndm, nsub, nfine, dm_list, p->s1, p->s2, p->nominal,
                                  p->maxshift2, p->max_delay);
@@ -325,7 +380,10 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaFree(p->d_s1);
         cudaFree(p->d_s2);
         cudaFree(p->d_maxshift2);
+        cudaFree(p->d_win_meta);
+        cudaFree(p->d_win_kfinal);
     }
+    p->pairs.release();
     p->scratch.release();
     p->host_in.release();
     p->host_out.release();
@@ -370,8 +428,8 @@ dedisp_status dedisp_plan_set_kernel(dedisp_plan* p, dedisp_kernel k)
 {
     if (!p || k < DEDISP_KERNEL_AUTO || k > DEDISP_KERNEL_WINDOW)
         return DEDISP_EINVAL;
-    if (k == DEDISP_KERNEL_WINDOW)
-        return DEDISP_ESTATE;  // not available for this plan
+    if (k == DEDISP_KERNEL_WINDOW && !(p->nsub == 0 && p->win.ok && p->win_fits))
+        return DEDISP_ESTATE;  // the shift table does not fit the register-window kernel's limits
     p->kernel = k;
     return DEDISP_OK;
 }
@@ -380,7 +438,24 @@ int dedisp_plan_resolved_kernel(const dedisp_plan* p, dedisp_dtype dtype)
 {
     if (!p || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
         return -1;
+    if (use_window(p, dtype))
+        return DEDISP_KERNEL_WINDOW;
     return p->kernel == DEDISP_KERNEL_AUTO ? DEDISP_KERNEL_DIRECT : p->kernel;
+}
+
+dedisp_status dedisp_plan_window_info(const dedisp_plan* p, int64_t* info)
+{
+    if (!p || !info)
+        return DEDISP_EINVAL;
+    info[0] = p->win.ok && p->win_fits;
+    info[1] = p->win.H;
+    info[2] = p->win.kmax;
+    info[3] = p->win.lmax;
+    info[4] = p->win.ntile_dm;
+    info[5] = kWinNS;
+    info[6] = kWinDB;
+    info[7] = p->win.maxbase;
+    return DEDISP_OK;
 }
 
 int64_t dedisp_plan_scratch_bytes(const dedisp_plan* p, int64_t nsamp_out, int nbeams)

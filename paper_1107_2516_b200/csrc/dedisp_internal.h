@@ -46,5 +46,49 @@ int launch_naive(const Problem& p, Elem in_t, void* stream, int* launches);
 // (max shift - min shift) inside a tile; decides how many rows share one staged copy.
 int launch_direct(const Problem& p, Elem in_t, const int spread[3], void* stream, int* launches);
 
+// ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
+// Geometry of the register-window kernel: a block owns kWinDB DM rows; warp (g, wt) owns the kWinD
+// rows of row group g and lanes own kWinT consecutive "slots" each, a slot being one pair of output
+// samples (t, t + H) of one row.  See DESIGN.md "Register-window kernel".
+constexpr int kWinD = 8;                          // DM rows per thread
+constexpr int kWinT = 10;                         // slots (sample pairs) per thread and row
+constexpr int kWinNG = 4;                         // row groups per block
+constexpr int kWinNT = 2;                         // warps along time per row group
+constexpr int kWinDB = kWinD * kWinNG;            // 32 DM rows per block
+constexpr int kWinNS = kWinNT * 32 * kWinT;       // 640 slots per row and block
+constexpr int kWinNW = 14;                        // register window, in pairs
+constexpr int kWinOMax = kWinNW - kWinT;          // largest row offset into the window (4)
+constexpr int kWinMetaWords = 12;                 // per (DM tile, channel) metadata, 48 bytes
+
+struct WindowPlan {
+    bool ok = false;
+    int H = 0;          // pairs (t, t+H): a block emits 2H samples per row
+    int kmax = 0;       // largest accumulated row skew
+    int lmax = 0;       // longest staged channel segment, in pairs
+    int ntile_dm = 0;
+    int64_t maxbase = 0;  // largest staged-segment start (in samples, relative to the tile start)
+    // meta[tile][c] = { base, len, wb[4], om[4], mask2, 0 }: staged segment start/length (pairs),
+    // per row group the window start (pairs, even) and 8 x 3-bit row offsets | shift mask << 24;
+    // mask2: a second shift of the same channel, one byte per row group
+    std::vector<int32_t> meta;
+    std::vector<int32_t> kfinal;  // [tile][32] final skew of every row
+};
+// shift: host table [ndm][nchans].  Returns false (wp.ok = false) when the table does not fit the
+// kernel's limits (non-monotone DMs, skew growing by more than one sample per channel, ...).
+bool build_window_plan(const int32_t* shift, int ndm, int nchans, WindowPlan& wp);
+
+struct WindowArgs {
+    const void* in;       // [nbeams][nchans][in_stride]
+    void* out;            // [nbeams][ndm][out_stride]
+    void* pairs;          // scratch [nbeams][nchans][pair_stride] float2
+    const int32_t* meta;  // device copies of WindowPlan::meta / kfinal
+    const int32_t* kfinal;
+    int64_t in_stride, out_stride, pair_stride, in_len, n_out;
+    int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t;
+};
+bool window_fits_smem(int lmax);  // the staging ring needs >= 8 slots of shared memory
+int64_t window_pair_stride(const WindowPlan& wp, int64_t n_out);  // float2 elements per channel row
+int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches);
+
 }  // namespace dedisp
 #endif
