@@ -127,10 +127,11 @@ DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel
 DEDISP_API int dedisp_plan_resolved_kernel(const dedisp_plan *plan, dedisp_dtype dtype);
 
 /* Geometry the register-window kernel would use for this plan, 8 int64 to HOST memory:
- * [0] 1 if the plan's table fits the kernel (else the rest is 0), [1] H: a block emits the sample
- * pairs (t, t+H), 2H samples per DM row, [2] largest accumulated row skew (slots lost per 640),
- * [3] longest staged channel segment in pairs, [4] DM tiles, [5] slots per row and block (640),
- * [6] DM rows per block (32), [7] largest segment start.  Brute-force plans only carry one. */
+ * [0] 1 if the plan's table fits the kernel (else the rest is 0), [1] H: a warp emits the sample
+ * pairs (t, t+H) of H consecutive t per DM row, [2] largest number of row shifts in a channel band
+ * (slots lost per warp tile), [3] longest staged channel segment in pairs, [4] DM tiles,
+ * [5] slots per row and warp, [6] DM rows per block, [7] channel bands (= kernel launches).
+ * Brute-force plans only carry one. */
 DEDISP_API dedisp_status dedisp_plan_window_info(const dedisp_plan *plan, int64_t *info);
 
 /* Bytes of device scratch a subband execute of nsamp_out samples and nbeams beams needs

@@ -143,7 +143,7 @@ class Plan:
         """dedisp_plan_window_info as a dict (geometry of the register-window kernel)."""
         a = np.zeros(8, dtype=np.int64)
         _check(lib().dedisp_plan_window_info(self._h, a.ctypes.data), "dedisp_plan_window_info")
-        keys = ("ok", "H", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "maxbase")
+        keys = ("ok", "H", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "nband")
         return dict(zip(keys, (int(v) for v in a)))
 
     def scratch_bytes(self, nsamp_out, nbeams=1):

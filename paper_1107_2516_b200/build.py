@@ -37,6 +37,9 @@ def build(force=False, verbose=False):
     """Compile every CUDA source of the package into LIB; returns its path."""
     if not force and not _stale():
         return LIB
+    gen, inc = os.path.join(CSRC, "gen_window_rows.py"), os.path.join(CSRC, "window_rows.inc")
+    if not os.path.exists(inc) or os.path.getmtime(inc) < os.path.getmtime(gen):
+        subprocess.check_call([sys.executable, gen])
     objs = []
     bdir = os.path.join(HERE, "build")
     os.makedirs(bdir, exist_ok=True)

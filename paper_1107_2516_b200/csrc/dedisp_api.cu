@@ -88,7 +88,7 @@ struct dedisp_plan {
     // register-window kernel (brute-force plans): host plan, device tables, pair scratch
     WindowPlan win;
     bool win_fits = false;
-    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr;
+    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr, *d_win_theta = nullptr;
     DevBuf pairs;
 };
 
@@ -129,6 +129,8 @@ dedisp_status upload(dedisp_plan* p)
             e = up(&p->d_win_meta, p->win.meta);
             if (e == cudaSuccess)
                 e = up(&p->d_win_kfinal, p->win.kfinal);
+            if (e == cudaSuccess)
+                e = up(&p->d_win_theta, p->win.theta);
         }
     } else {
         e = up(&p->d_s1, p->s1);
@@ -173,6 +175,10 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.pairs = plan->pairs.p;
     a.meta = plan->d_win_meta;
     a.kfinal = plan->d_win_kfinal;
+    a.theta = plan->d_win_theta;
+    a.nband = plan->win.nband;
+    a.band = plan->win.band.data();
+    a.geom = plan->win.geom;
     a.in_stride = in_stride;
     a.out_stride = out_stride;
     a.in_len = nsamp_out + plan->max_delay;
@@ -183,7 +189,7 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.H = plan->win.H;
     a.lmax = plan->win.lmax;
     a.ntile_dm = plan->win.ntile_dm;
-    a.ntile_t = static_cast<int>((nsamp_out + 2 * plan->win.H - 1) / (2 * plan->win.H));
+    a.ntile_t = static_cast<int>(window_ntile_t(plan->win, nsamp_out));
     return launch_window(a, in_t, stream, &plan->last_launches) == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
@@ -342,8 +348,8 @@ dedisp_status dedisp_plan_create(dedisp_plan** plan, int nchans, double f_top_mh
         if (nsub == 0) {
             for (int k = 0; k < 3; ++k)
                 p->spread_full[k] = tile_spread(p->shift.data(), ndm, nchans, nchans, tiles[k]);
-            build_window_plan(p->shift.data(), ndm, nchans, p->win);
-            p->win_fits = p->win.ok && window_fits_smem(p->win.lmax);
+            build_window_plan(p->shift.data(), ndm, nchans, window_default_geom(), p->win);
+            p->win_fits = p->win.ok && window_fits_smem(p->win);
         } else {
             build_subband_tables(p->shift, nchans, ndm, nsub, nfine, dm_list, p->s1, p->s2, p->nominal,
                                  p->maxshift2, p->max_delay);
@@ -382,6 +388,7 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaFree(p->d_maxshift2);
         cudaFree(p->d_win_meta);
         cudaFree(p->d_win_kfinal);
+        cudaFree(p->d_win_theta);
     }
     p->pairs.release();
     p->scratch.release();
@@ -452,9 +459,9 @@ dedisp_status dedisp_plan_window_info(const dedisp_plan* p, int64_t* info)
     info[2] = p->win.kmax;
     info[3] = p->win.lmax;
     info[4] = p->win.ntile_dm;
-    info[5] = kWinNS;
-    info[6] = kWinDB;
-    info[7] = p->win.maxbase;
+    info[5] = p->win.geom.W();
+    info[6] = p->win.geom.rows();
+    info[7] = p->win.nband;
     return DEDISP_OK;
 }
 

@@ -47,48 +47,61 @@ int launch_naive(const Problem& p, Elem in_t, void* stream, int* launches);
 int launch_direct(const Problem& p, Elem in_t, const int spread[3], void* stream, int* launches);
 
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
-// Geometry of the register-window kernel: a block owns kWinDB DM rows; warp (g, wt) owns the kWinD
-// rows of row group g and lanes own kWinT consecutive "slots" each, a slot being one pair of output
-// samples (t, t + H) of one row.  See DESIGN.md "Register-window kernel".
-constexpr int kWinD = 8;                          // DM rows per thread
-constexpr int kWinT = 10;                         // slots (sample pairs) per thread and row
-constexpr int kWinNG = 4;                         // row groups per block
-constexpr int kWinNT = 2;                         // warps along time per row group
-constexpr int kWinDB = kWinD * kWinNG;            // 32 DM rows per block
-constexpr int kWinNS = kWinNT * 32 * kWinT;       // 640 slots per row and block
-constexpr int kWinNW = 14;                        // register window, in pairs
-constexpr int kWinOMax = kWinNW - kWinT;          // largest row offset into the window (4)
-constexpr int kWinMetaWords = 12;                 // per (DM tile, channel) metadata, 48 bytes
+// Geometry: a consumer warp owns the kWinD = 8 DM rows of one
+// row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
+// pair of output samples (t, t + NT*H).  A block has G row groups x NT warps along time
+// (+ 1 producer warp); the channel loop is cut into bands, one launch per band.
+constexpr int kWinD = 8;            // DM rows per thread
+constexpr int kWinMetaWords = 16;   // per (DM tile, channel) metadata, 64 bytes
+constexpr int kWinWbBits = 11;      // window offset inside the staged segment, in pairs
+
+struct WindowGeom {
+    int T = 0;   // slots per lane and row (odd: conflict-free LDS.64)
+    int G = 0;   // row groups per block (<= 8)
+    int NT = 0;  // warps along time per row group
+    int W() const { return 32 * T; }
+    int rows() const { return kWinD * G; }
+};
 
 struct WindowPlan {
     bool ok = false;
-    int H = 0;          // pairs (t, t+H): a block emits 2H samples per row
-    int kmax = 0;       // largest accumulated row skew
+    WindowGeom geom;
+    int H = 0;          // output samples per warp, row and half pair: W - kmax
+    int kmax = 0;       // largest number of row shifts of a row inside one band
     int lmax = 0;       // longest staged channel segment, in pairs
     int ntile_dm = 0;
-    int64_t maxbase = 0;  // largest staged-segment start (in samples, relative to the tile start)
-    // meta[tile][c] = { base, len, wb[4], om[4], mask2, 0 }: staged segment start/length (pairs),
-    // per row group the window start (pairs, even) and 8 x 3-bit row offsets | shift mask << 24;
-    // mask2: a second shift of the same channel, one byte per row group
+    int nband = 0;
+    int theta_max = 0;  // largest band skew of a row
+    int64_t maxbase = 0;        // largest staged-segment start (pairs, relative to the tile start)
+    std::vector<int32_t> band;  // [nband + 1] channel boundaries
+    // meta[tile][c] = { base, len, m[G], 0.. }: staged segment start / length in pairs (both even)
+    // and, per row group, jitter bits (rows 1..7) | shift mask << 7 | 2nd shift mask << 14 |
+    // window offset << 21
     std::vector<int32_t> meta;
-    std::vector<int32_t> kfinal;  // [tile][32] final skew of every row
+    std::vector<int32_t> kfinal;  // [tile][band][rows] row shifts of every row at the band's end
+    std::vector<int32_t> theta;   // [tile][band][rows] band skew of every row
 };
 // shift: host table [ndm][nchans].  Returns false (wp.ok = false) when the table does not fit the
-// kernel's limits (non-monotone DMs, skew growing by more than one sample per channel, ...).
-bool build_window_plan(const int32_t* shift, int ndm, int nchans, WindowPlan& wp);
+// kernel's limits (non-monotone DMs, neighbouring trials drifting apart too fast, ...).
+bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGeom& g, WindowPlan& wp);
 
 struct WindowArgs {
     const void* in;       // [nbeams][nchans][in_stride]
     void* out;            // [nbeams][ndm][out_stride]
     void* pairs;          // scratch [nbeams][nchans][pair_stride] float2
-    const int32_t* meta;  // device copies of WindowPlan::meta / kfinal
+    const int32_t* meta;  // device copies of WindowPlan::meta / kfinal / theta
     const int32_t* kfinal;
+    const int32_t* theta;
     int64_t in_stride, out_stride, pair_stride, in_len, n_out;
-    int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t;
+    int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t, nband;
+    const int32_t* band;  // HOST pointer, [nband + 1]
+    WindowGeom geom;
 };
-bool window_fits_smem(int lmax);  // the staging ring needs >= 8 slots of shared memory
+bool window_fits_smem(const WindowPlan& wp);
+int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out);
 int64_t window_pair_stride(const WindowPlan& wp, int64_t n_out);  // float2 elements per channel row
 int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches);
+WindowGeom window_default_geom();
 
 }  // namespace dedisp
 #endif

@@ -2,19 +2,22 @@
 //
 //   out[d][t] = sum_c in[c][t + shift(c,d)]
 //
-// Two launches per execute:
-//  1. pairify_kernel: P[c][u] = (in[c][u], in[c][u+H]) as float2 (uint8 input is widened to fp32
-//     here; sums of <= 2^24/255 bytes are exact in fp32).  Pairing two samples H apart that share
-//     (c, d) and therefore the same shift lets the main kernel add two outputs per instruction
+// Launches per execute: one pairify, then one window_kernel per channel band.
+//  1. pairify_kernel: P[c][u] = (in[c][u], in[c][u + NT*H]) as float2 (uint8 input is widened to
+//     fp32 here; sums of < 2^24/255 bytes are exact in fp32).  Two samples NT*H apart that share
+//     (c, d) have the same shift, so the main kernel adds two outputs per instruction
 //     (add.f32x2 -> FADD2) from naturally aligned 64-bit registers, whatever the shift's parity.
-//  2. window_kernel: one block = 32 DM rows x 2H output samples.  A thread keeps 8 rows x 10 pairs
-//     of accumulators in registers for the whole channel loop; per channel it loads ONE window of
-//     14 staged pairs (7 LDS.128) that feeds all 8 rows (row j starts 0..4 pairs into the window,
-//     a warp-uniform 5-way branch selects the unrolled variant).  Rows keep up with the growing
-//     delay difference between neighbouring DM trials by occasionally moving their accumulators up
-//     one slot ("row shift", planned on the host: window_plan.cpp).  Channel segments are staged
-//     into a ring of shared-memory slots by 1-D TMA bulk copies (cp.async.bulk + mbarrier) issued
-//     by one thread, so the compute warps spend no instructions or registers on staging.
+//  2. window_kernel (band b): a block = G row groups x NT warps; a consumer
+//     warp owns 8 DM rows x 32*T slots (pairs of output samples) and keeps their 8 x T packed
+//     accumulators in registers for the whole band.  Per channel it loads ONE window of T + 1
+//     staged pairs (LDS.64, conflict-free for odd T) that feeds all 8 rows: row j adds
+//     w[i + o_j], o_j in {0, 1} chosen by a warp-uniform two-way branch (window_rows.inc).  Rows
+//     follow the growing delay difference between neighbouring DM trials by moving their
+//     accumulators up one slot now and then ("row shift", planned on the host: window_plan.cpp).
+//     Channel segments are staged into a ring of shared-memory slots by 1-D TMA bulk copies
+//     (cp.async.bulk + mbarrier) issued by thread 0 a few channels ahead.  At the end of the band the
+//     accumulators go through a per-warp shared-memory transpose to coalesced global accesses:
+//     band 0 stores, later bands add to what is there.
 #include <cuda_runtime.h>
 
 #include "dedisp_internal.h"
@@ -29,7 +32,7 @@ typedef unsigned long long u64;
 template <typename InT>
 __global__ void __launch_bounds__(256) pairify_kernel(const InT* __restrict__ in, float2* __restrict__ pairs,
                                                       int64_t in_stride, int64_t pair_stride,
-                                                      int64_t in_len, int H)
+                                                      int64_t in_len, int hp)
 {
     const int64_t u = (static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x) * 2;
     if (u >= pair_stride)
@@ -39,7 +42,7 @@ __global__ void __launch_bounds__(256) pairify_kernel(const InT* __restrict__ in
     float v[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const int64_t idx = u + (k & 1) + (k >> 1) * static_cast<int64_t>(H);
+        const int64_t idx = u + (k & 1) + (k >> 1) * static_cast<int64_t>(hp);
         v[k] = idx < in_len ? static_cast<float>(src[idx]) : 0.0f;
     }
     // pair_stride is even and the scratch is 16-byte aligned
@@ -89,173 +92,182 @@ __device__ __forceinline__ u64 add2(u64 a, u64 b)
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
-__device__ __forceinline__ void named_bar(int id, int nthreads)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
-}
+
+#include "window_rows.inc"
 
 // ------------------------------------------------------------------------------------------------
 // 2. window kernel
 // ------------------------------------------------------------------------------------------------
-constexpr int kWinThreads = kWinNG * kWinNT * 32;  // 256
-constexpr int kSlotHdr = 64;                       // bytes of metadata in front of a staged segment
-constexpr int kLag = 4;                            // the producer refills the slot used kLag channels ago
+constexpr int kSlotHdr = kWinMetaWords * 4;  // bytes of metadata in front of a staged segment
 
-template <int O> __device__ __forceinline__ void add_row(u64 (&acc)[kWinT], const u64 (&w)[kWinNW])
+// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one
+template <int T> __device__ __forceinline__ void shift_rows(u64 (&acc)[kWinD][T], unsigned mask, int lane)
 {
 #pragma unroll
-    for (int i = 0; i < kWinT; ++i)
-        acc[i] = add2(acc[i], w[O + i]);
+    for (int j = 1; j < kWinD; ++j) {
+        if (mask & (1u << (j - 1))) {
+            const u64 carry = __shfl_up_sync(0xffffffffu, acc[j][T - 1], 1);
+#pragma unroll
+            for (int i = T - 1; i > 0; --i)
+                acc[j][i] = acc[j][i - 1];
+            acc[j][0] = lane ? carry : 0ull;
+        }
+    }
 }
 
-// smem layout: [nslot] full barriers | [nslot] empty barriers | mailbox [NG][D] u64 | slots
-template <typename OutT>
-__global__ void __launch_bounds__(kWinThreads, 1) window_kernel(const WindowArgs a, const int nslot,
-                                                                 const int slot_bytes)
+template <int T> __device__ __forceinline__ void load_window(u64 (&w)[T + 1], const unsigned char* p)
 {
+    const u64* q = reinterpret_cast<const u64*>(p);
+#pragma unroll
+    for (int k = 0; k <= T; ++k)
+        w[k] = q[k];
+}
+
+__device__ __forceinline__ void put(float* p, float v, bool first) { *p = first ? v : *p + v; }
+// int32 output: the fp32 partial sums are exact integers (nchans * 255 < 2^24)
+__device__ __forceinline__ void put(int32_t* p, float v, bool first)
+{
+    const int iv = __float2int_rn(v);
+    *p = first ? iv : *p + iv;
+}
+
+// smem layout: [nslot] full barriers | [nslot] empty barriers | transpose scratch [NCW][W] u64 | slots
+template <int T, int G, int NT, typename OutT>
+__global__ void __launch_bounds__(G * NT * 32, 1)
+    window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int nslot_log2,
+                  const int slot_bytes)
+{
+    constexpr int W = 32 * T, NCW = G * NT, RB = kWinD * G;
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int g = warp / kWinNT, wt = warp % kWinNT;
     const int ty = blockIdx.x, beam = blockIdx.z;
-    const int64_t tb0 = static_cast<int64_t>(blockIdx.y) * 2 * a.H;
+    const int64_t T0 = static_cast<int64_t>(blockIdx.y) * 2 * NT * a.H;
+    const int nslot = 1 << nslot_log2;
 
     const unsigned bar_full = smem_u32(smem);
     const unsigned bar_empty = bar_full + 8u * nslot;
-    u64* mailbox = reinterpret_cast<u64*>(smem + 16 * nslot);
-    const int slots_off = (16 * nslot + kWinNG * kWinD * 8 + 127) & ~127;
+    const int tr_off = (16 * nslot + 127) & ~127;
+    const int slots_off = (tr_off + NCW * W * 8 + 127) & ~127;
     unsigned char* slots = smem + slots_off;
 
     if (tid == 0) {
         for (int s = 0; s < nslot; ++s) {
             mbar_init(bar_full + 8u * s, 1);
-            mbar_init(bar_empty + 8u * s, kWinNG * kWinNT);
+            mbar_init(bar_empty + 8u * s, NCW);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    const int32_t* meta = a.meta + static_cast<int64_t>(ty) * a.nchans * kWinMetaWords;
-    const float2* prow = static_cast<const float2*>(a.pairs) + static_cast<int64_t>(beam) * a.nchans * a.pair_stride + tb0;
+    const int nch = c_end - c_begin;
+    const int32_t* meta = a.meta + (static_cast<int64_t>(ty) * a.nchans + c_begin) * kWinMetaWords;
 
-    // producer state (warp 0, lane 0 only)
-    const bool producer = tid == 0;
-    int cp = 0;  // next channel to stage
-    auto produce = [&](int c) {
-        const int s = c % nslot;
-        const int32_t* m = meta + static_cast<int64_t>(c) * kWinMetaWords;
+    // ---- producer duty (thread 0): stage channel i into slot i % nslot, kLead channels ahead ------------
+    const float2* prow = static_cast<const float2*>(a.pairs) +
+                         (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
+    const int64_t pair_stride = a.pair_stride;
+    auto produce = [&](int i) {
+        const int s = i & (nslot - 1), lap = i >> nslot_log2;
+        if (lap > 0)
+            mbar_wait(bar_empty + 8u * s, (lap - 1) & 1);
+        const int32_t* m = meta + static_cast<int64_t>(i) * kWinMetaWords;
         const int base = __ldg(m), len = __ldg(m + 1);
         const unsigned dst = smem_u32(slots + static_cast<size_t>(s) * slot_bytes);
         const unsigned fb = bar_full + 8u * s;
-        mbar_expect_tx(fb, kWinMetaWords * 4 + len * 8);
-        bulk_g2s(dst, m, kWinMetaWords * 4, fb);
-        bulk_g2s(dst + kSlotHdr, prow + static_cast<int64_t>(c) * a.pair_stride + base, len * 8, fb);
+        mbar_expect_tx(fb, kSlotHdr + len * 8);
+        bulk_g2s(dst, m, kSlotHdr, fb);
+        bulk_g2s(dst + kSlotHdr, prow + static_cast<int64_t>(i) * pair_stride + base, len * 8, fb);
     };
-    if (producer) {
-        const int n0 = min(nslot - kLag, a.nchans);
-        for (; cp < n0; ++cp)
-            produce(cp);
-    }
+    const int lead = nslot - 4;
+    const bool producer = tid == 0;
+    if (producer)
+        for (int i = 0; i < lead && i < nch; ++i)
+            produce(i);
 
-    u64 acc[kWinD][kWinT];
+    // ---- consumers ------------------------------------------------------------------------------------
+    const int g = warp / NT, wt = warp % NT;
+    u64 acc[kWinD][T];
 #pragma unroll
     for (int j = 0; j < kWinD; ++j)
 #pragma unroll
-        for (int i = 0; i < kWinT; ++i)
+        for (int i = 0; i < T; ++i)
             acc[j][i] = 0ull;
 
-    const int p0 = (wt * 32 + lane) * kWinT;  // first slot of this thread
+    const int lane_off = kSlotHdr + (wt * a.H + lane * T) * 8;  // bytes from the slot start
+    auto slot_ptr = [&](int i) { return slots + static_cast<size_t>(i & (nslot - 1)) * slot_bytes; };
+    auto wait_full = [&](int i) { mbar_wait(bar_full + 8u * (i & (nslot - 1)), (i >> nslot_log2) & 1); };
+    auto slot_word = [&](int i) { return reinterpret_cast<const unsigned*>(slot_ptr(i))[2 + g]; };
 
-    for (int c = 0; c < a.nchans; ++c) {
-        const int s = c % nslot;
-        const unsigned ph = (c / nslot) & 1;
-        if (producer && cp < a.nchans) {
-            // slot of channel cp was last used by channel cp - nslot (<= c - kLag)
-            if (cp >= nslot)
-                mbar_wait(bar_empty + 8u * (cp % nslot), ((cp / nslot) - 1) & 1);
-            produce(cp);
-            ++cp;
-        }
-        mbar_wait(bar_full + 8u * s, ph);
-        const unsigned char* slot = slots + static_cast<size_t>(s) * slot_bytes;
-        const int wb = reinterpret_cast<const int*>(slot)[2 + g];
-        const unsigned om = reinterpret_cast<const unsigned*>(slot)[6 + g];
+    // software pipeline: channel i is added from w/m while the window of i+1 and the metadata of
+    // i+2 are on their way
+    u64 wa[T + 1], wb[T + 1];
+    unsigned m = 0, mn = 0, mnn = 0;
+    wait_full(0);
+    m = slot_word(0);
+    if (nch > 1) {
+        wait_full(1);
+        mn = slot_word(1);
+    }
+    load_window<T>(wa, slot_ptr(0) + lane_off + (m >> 21) * 8);
 
-        // row shifts (uniform over the two warps of this row group): the accumulators of the rows
-        // in the mask move up one slot; the pair leaving lane 31 of the first warp reaches lane 0
-        // of the second through the mailbox
-        unsigned mask = om >> 24;
-        if (mask) {
-            const unsigned mask2 = (reinterpret_cast<const unsigned*>(slot)[10] >> (8 * g)) & 0xffu;
-            for (int pass = 0; pass < 2 && mask; ++pass) {
-                if (wt == 0 && lane == 31) {
-#pragma unroll
-                    for (int j = 1; j < kWinD; ++j)
-                        if (mask & (1u << j))
-                            mailbox[g * kWinD + j] = acc[j][kWinT - 1];
-                }
-                named_bar(1 + g, kWinNT * 32);
-#pragma unroll
-                for (int j = 1; j < kWinD; ++j) {
-                    if (mask & (1u << j)) {
-                        u64 carry = __shfl_up_sync(0xffffffffu, acc[j][kWinT - 1], 1);
-                        if (lane == 0)
-                            carry = wt ? mailbox[g * kWinD + j] : 0ull;
-#pragma unroll
-                        for (int i = kWinT - 1; i > 0; --i)
-                            acc[j][i] = acc[j][i - 1];
-                        acc[j][0] = carry;
-                    }
-                }
-                named_bar(1 + g, kWinNT * 32);
-                mask = mask2;
-            }
+    auto step = [&](int i, u64(&w)[T + 1], u64(&wn)[T + 1]) {
+        if (producer && i + lead < nch)
+            produce(i + lead);
+        if (i + 1 < nch)
+            load_window<T>(wn, slot_ptr(i + 1) + lane_off + (mn >> 21) * 8);
+        if (i + 2 < nch) {
+            wait_full(i + 2);
+            mnn = slot_word(i + 2);
         }
-
-        u64 w[kWinNW];
-        const ulonglong2* wp = reinterpret_cast<const ulonglong2*>(slot + kSlotHdr + static_cast<size_t>(p0 + wb) * 8);
-#pragma unroll
-        for (int k = 0; k < kWinNW / 2; ++k) {
-            const ulonglong2 v = wp[k];
-            w[2 * k] = v.x;
-            w[2 * k + 1] = v.y;
+        const unsigned sm = (m >> 7) & 0x3fffu;
+        if (sm) {
+            shift_rows<T>(acc, sm & 127u, lane);
+            if (sm >> 7)
+                shift_rows<T>(acc, sm >> 7, lane);
         }
 #pragma unroll
-        for (int j = 0; j < kWinD; ++j) {
-            switch ((om >> (3 * j)) & 7u) {
-            case 0: add_row<0>(acc[j], w); break;
-            case 1: add_row<1>(acc[j], w); break;
-            case 2: add_row<2>(acc[j], w); break;
-            case 3: add_row<3>(acc[j], w); break;
-            default: add_row<4>(acc[j], w); break;
-            }
-        }
+        for (int k = 0; k < T; ++k)
+            acc[0][k] = add2(acc[0][k], w[k]);
+        rows7(acc, w, m);
         __syncwarp();
         if (lane == 0)
-            mbar_arrive(bar_empty + 8u * s);
+            mbar_arrive(bar_empty + 8u * (i & (nslot - 1)));
+        m = mn;
+        mn = mnn;
+    };
+#pragma unroll 1
+    for (int i = 0; i < nch; i += 2) {
+        step(i, wa, wb);
+        if (i + 1 < nch)
+            step(i + 1, wb, wa);
     }
 
-    // epilogue: slot p of row j is output time p - kfinal_j (valid in [0, H)), pair = (t, t + H)
+    // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
+    u64* tr = reinterpret_cast<u64*>(smem + tr_off) + warp * W;
+    const bool first = band == 0;
+    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
+    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
     OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
+    const int64_t hp = static_cast<int64_t>(NT) * a.H;
 #pragma unroll
     for (int j = 0; j < kWinD; ++j) {
-        const int r = g * kWinD + j;
-        const int d = ty * kWinDB + r;
-        if (d >= a.ndm)
-            continue;
-        const int kf = __ldg(a.kfinal + ty * kWinDB + r);
-        OutT* o = out + static_cast<int64_t>(d) * a.out_stride;
+        const int d = ty * RB + g * kWinD + j;
+        __syncwarp();
 #pragma unroll
-        for (int i = 0; i < kWinT; ++i) {
-            const int tl = p0 + i - kf;
-            if (tl < 0 || tl >= a.H)
-                continue;
-            const int64_t t = tb0 + tl;
-            const float lo = __uint_as_float(static_cast<unsigned>(acc[j][i]));
-            const float hi = __uint_as_float(static_cast<unsigned>(acc[j][i] >> 32));
-            if (t < a.n_out)
-                o[t] = static_cast<OutT>(lo);
-            if (t + a.H < a.n_out)
-                o[t + a.H] = static_cast<OutT>(hi);
+        for (int i = 0; i < T; ++i)
+            tr[lane * T + i] = acc[j][i];
+        __syncwarp();
+        if (d < a.ndm) {
+            const int kf = __ldg(kfp + j), th = __ldg(thp + j);
+            OutT* o = out + static_cast<int64_t>(d) * a.out_stride;
+            for (int q = lane; q < a.H; q += 32) {
+                const u64 v = tr[q + kf];
+                const int64_t t = T0 + wt * a.H + q - th;
+                if (t >= 0 && t < a.n_out)
+                    put(o + t, __uint_as_float(static_cast<unsigned>(v)), first);
+                if (t + hp >= 0 && t + hp < a.n_out)
+                    put(o + t + hp, __uint_as_float(static_cast<unsigned>(v >> 32)), first);
+            }
         }
     }
 }
@@ -263,21 +275,61 @@ __global__ void __launch_bounds__(kWinThreads, 1) window_kernel(const WindowArgs
 // ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
-static int window_ring(int lmax, int* slot_bytes)
+static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes, int* nslot_log2)
 {
     const int sb = (kSlotHdr + lmax * 8 + 127) & ~127;
-    const int budget = 227 * 1024 - 1024;
-    int nslot = budget / sb;
-    if (nslot > 32)
-        nslot = 32;
+    const int fixed = 256 + g.G * g.NT * g.W() * 8 + 256;
+    const int budget = 227 * 1024 - fixed;
+    int lg = 4;  // at most 16 slots
+    while (lg > 3 && (sb << lg) > budget)
+        --lg;
     *slot_bytes = sb;
-    return nslot;
+    *nslot_log2 = lg;
+    return (sb << lg) <= budget ? (1 << lg) : 0;
 }
 
-bool window_fits_smem(int lmax)
+bool window_fits_smem(const WindowPlan& wp)
 {
-    int sb;
-    return window_ring(lmax, &sb) >= 2 * kLag;
+    int sb, lg;
+    return wp.ok && window_ring(wp.geom, wp.lmax, &sb, &lg) >= 8;
+}
+
+template <int T, int G, int NT, typename OutT>
+static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
+{
+    int slot_bytes = 0, lg = 0;
+    const int nslot = window_ring(a.geom, a.lmax, &slot_bytes, &lg);
+    if (nslot < 8)
+        return static_cast<int>(cudaErrorInvalidConfiguration);
+    const int tr_off = (16 * nslot + 127) & ~127;
+    const int slots_off = (tr_off + G * NT * 32 * T * 8 + 127) & ~127;
+    const size_t smem = static_cast<size_t>(slots_off) + static_cast<size_t>(nslot) * slot_bytes;
+    cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(smem));
+    if (e != cudaSuccess)
+        return static_cast<int>(e);
+    dim3 grid(a.ntile_dm, a.ntile_t, a.nbeams);
+    for (int b = 0; b < a.nband; ++b) {
+        window_kernel<T, G, NT, OutT><<<grid, G * NT * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b, lg,
+                                                                              slot_bytes);
+        ++*launches;
+        e = cudaGetLastError();
+        if (e != cudaSuccess)
+            return static_cast<int>(e);
+    }
+    return 0;
+}
+
+template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_t st, int* launches)
+{
+    const WindowGeom& g = a.geom;
+    if (g.T == 9 && g.G == 8 && g.NT == 1)
+        return launch_bands<9, 8, 1, OutT>(a, st, launches);
+    if (g.T == 5 && g.G == 8 && g.NT == 2)
+        return launch_bands<5, 8, 2, OutT>(a, st, launches);
+    if (g.T == 7 && g.G == 4 && g.NT == 3)
+        return launch_bands<7, 4, 3, OutT>(a, st, launches);
+    return static_cast<int>(cudaErrorInvalidConfiguration);
 }
 
 int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
@@ -285,42 +337,20 @@ int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
     if (a.n_out <= 0 || a.ndm <= 0)
         return 0;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    int slot_bytes = 0;
-    const int nslot = window_ring(a.lmax, &slot_bytes);
-    if (nslot < 2 * kLag)
-        return static_cast<int>(cudaErrorInvalidConfiguration);
-    const int slots_off = (16 * nslot + kWinNG * kWinD * 8 + 127) & ~127;
-    const size_t smem = static_cast<size_t>(slots_off) + static_cast<size_t>(nslot) * slot_bytes;
-
     dim3 pgrid(static_cast<unsigned>((a.pair_stride / 2 + 255) / 256), a.nchans, a.nbeams);
     float2* pairs = static_cast<float2*>(a.pairs);
+    const int hp = a.geom.NT * a.H;
     if (in_t == Elem::F32)
         pairify_kernel<float><<<pgrid, 256, 0, st>>>(static_cast<const float*>(a.in), pairs, a.in_stride,
-                                                     a.pair_stride, a.in_len, a.H);
+                                                     a.pair_stride, a.in_len, hp);
     else
         pairify_kernel<uint8_t><<<pgrid, 256, 0, st>>>(static_cast<const uint8_t*>(a.in), pairs, a.in_stride,
-                                                       a.pair_stride, a.in_len, a.H);
+                                                       a.pair_stride, a.in_len, hp);
     ++*launches;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess)
         return static_cast<int>(e);
-
-    dim3 grid(a.ntile_dm, a.ntile_t, a.nbeams);
-    if (in_t == Elem::F32) {
-        e = cudaFuncSetAttribute(window_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 static_cast<int>(smem));
-        if (e != cudaSuccess)
-            return static_cast<int>(e);
-        window_kernel<float><<<grid, kWinThreads, smem, st>>>(a, nslot, slot_bytes);
-    } else {
-        e = cudaFuncSetAttribute(window_kernel<int32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 static_cast<int>(smem));
-        if (e != cudaSuccess)
-            return static_cast<int>(e);
-        window_kernel<int32_t><<<grid, kWinThreads, smem, st>>>(a, nslot, slot_bytes);
-    }
-    ++*launches;
-    return static_cast<int>(cudaGetLastError());
+    return in_t == Elem::F32 ? launch_geom<float>(a, st, launches) : launch_geom<int32_t>(a, st, launches);
 }
 
 }  // namespace dedisp

@@ -1,15 +1,19 @@
 // Host planner of the register-window kernel (kernels_window.cu).
 //
-// The kernel keeps, per thread, kWinD DM rows x kWinT output pairs in registers for the whole
-// channel loop and feeds all rows from ONE register window of kWinNW consecutive staged samples.
-// That only works if, for every channel c, the samples the kWinD rows need start within
-// kWinOMax positions of each other.  Neighbouring DM trials drift apart as the channel frequency
-// drops (eq. 1: the delay difference between two DMs grows like f^-2), so each row
-// j of a row group carries a skew kappa_j(c): slot p of row j stands for output time p - kappa_j.
-// kappa_j only ever grows, one sample at a time ("row shift": the row's accumulators move up one
-// slot), and is chosen lazily here so that
-//     0 <= [s(c,d_j) - kappa_j(c)] - s(c,d_0) <= 3      for every channel c
-// (at most two shifts of a row per channel).
+// A thread keeps kWinD = 8 DM rows x T output pairs in registers and feeds all rows from ONE
+// register window of T + 1 consecutive staged pairs per channel: row j adds w[i + o_j] to its
+// accumulator i, o_j in {0, 1}.  That needs, for every channel c, the samples of the 8 rows to start
+// within one position of a common base.  Neighbouring DM trials drift apart as the frequency drops
+// (eq. 1: the delay difference of two DMs grows like f^-2) and the rounded delays
+// dither by +-1 around that drift, so
+//   * row 0 of a row group is the reference: the window starts at its shift s_0(c);
+//   * row j carries base_j(c) = theta_j + kappa_j(c), non-decreasing in c, with
+//         o_j(c) = [s_j(c) - s_0(c)] - base_j(c)  in {0, 1};
+//     slot p of row j stands for output time  tile_start + p - base_j(c);
+//   * kappa_j grows one at a time ("row shift": the row's accumulators move up one slot) and every
+//     slot lost that way shortens the useful tile, so the channel loop is cut into BANDS: inside a
+//     band kappa_j <= kcap; a new band restarts with kappa = 0 and a fresh skew theta_j, and its
+//     partial sums are added to the output by a later launch (kernels_window.cu).
 // Everything the kernel needs per (DM tile, channel) is precomputed into WindowPlan::meta.
 #include <algorithm>
 #include <cstring>
@@ -18,102 +22,173 @@
 
 namespace dedisp {
 
-bool build_window_plan(const int32_t* shift, int ndm, int nchans, WindowPlan& wp)
+WindowGeom window_default_geom()
+{
+    WindowGeom g;
+    g.T = 9;
+    g.G = 8;
+    g.NT = 1;
+    return g;
+}
+
+namespace {
+
+struct Rows {
+    const int32_t* shift;
+    int ndm, nchans, RB;
+    const int32_t* row(int tile, int r) const
+    {
+        const int d = std::min(tile * RB + r, ndm - 1);  // tail rows repeat the last trial
+        return shift + static_cast<size_t>(d) * nchans;
+    }
+};
+
+}  // namespace
+
+bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGeom& geom, WindowPlan& wp)
 {
     wp = WindowPlan();
-    if (ndm <= 0 || nchans <= 0)
+    wp.geom = geom;
+    if (ndm <= 0 || nchans <= 0 || geom.T <= 0 || geom.G <= 0 || geom.G > 8 || geom.NT <= 0)
         return false;
-    const int ntile = (ndm + kWinDB - 1) / kWinDB;
-    wp.ntile_dm = ntile;
-    wp.meta.assign(static_cast<size_t>(ntile) * nchans * kWinMetaWords, 0);
-    wp.kfinal.assign(static_cast<size_t>(ntile) * kWinDB, 0);
-    int kmax = 0, lmax = 0;
-    int64_t maxbase = 0;
-    for (int ty = 0; ty < ntile; ++ty) {
-        const int32_t* rows[kWinDB];
-        for (int r = 0; r < kWinDB; ++r) {
-            const int d = std::min(ty * kWinDB + r, ndm - 1);  // tail rows repeat the last trial
-            rows[r] = shift + static_cast<size_t>(d) * nchans;
+    const int RB = geom.rows(), W = geom.W(), G = geom.G;
+    const int ntile = (ndm + RB - 1) / RB;
+    const int kcap = std::max(4, W / 16);
+    const Rows R{shift, ndm, nchans, RB};
+    const size_t nrow = static_cast<size_t>(ntile) * RB;
+
+    // ---- pass 1: band boundaries, common to all DM tiles ------------------------------------------
+    std::vector<int32_t> base(nrow), theta(nrow), nb(nrow);
+    std::vector<const int32_t*> rp(nrow), r0(nrow);
+    for (int ty = 0; ty < ntile; ++ty)
+        for (int r = 0; r < RB; ++r) {
+            rp[static_cast<size_t>(ty) * RB + r] = R.row(ty, r);
+            r0[static_cast<size_t>(ty) * RB + r] = R.row(ty, r / kWinD * kWinD);
         }
-        int kappa[kWinDB];
-        std::memset(kappa, 0, sizeof(kappa));
-        for (int c = 0; c < nchans; ++c) {
-            int32_t* m = wp.meta.data() + (static_cast<size_t>(ty) * nchans + c) * kWinMetaWords;
-            int raw0[kWinNG];
-            unsigned mask[kWinNG], mask2[kWinNG];
-            int64_t base = INT64_MAX;
-            for (int g = 0; g < kWinNG; ++g) {
-                const int s0 = rows[g * kWinD][c];
-                mask[g] = mask2[g] = 0;
-                for (int j = 1; j < kWinD; ++j) {
-                    int& k = kappa[g * kWinD + j];
-                    int diff = rows[g * kWinD + j][c] - s0 - k;
-                    // the row shifts by one slot (twice if need be) before this channel is added;
-                    // shifting at 3 already leaves room for the +-1 dither of the rounded delays
-                    if (diff > 2) {
-                        ++k;
-                        --diff;
-                        mask[g] |= 1u << j;
-                    }
-                    if (diff > 2) {
-                        ++k;
-                        --diff;
-                        mask2[g] |= 1u << j;
-                    }
-                    if (diff < 0 || diff > 3)
-                        return false;
-                }
-                raw0[g] = s0;
-                base = std::min<int64_t>(base, s0);
-            }
-            base &= ~static_cast<int64_t>(1);  // staged segments start on an even sample
-            int wbmax = 0;
-            for (int g = 0; g < kWinNG; ++g) {
-                const int e0 = static_cast<int>(raw0[g] - base);
-                const int wb = e0 & ~1;  // even: 16-byte aligned LDS.128 of two pairs
-                if (wb > 0xffffff)
-                    return false;
-                unsigned om = 0;
-                for (int j = 0; j < kWinD; ++j) {
-                    const int o = rows[g * kWinD + j][c] - kappa[g * kWinD + j] - static_cast<int>(base) - wb;
-                    if (o < 0 || o > kWinOMax)
-                        return false;
-                    om |= static_cast<unsigned>(o) << (3 * j);
-                }
-                om |= mask[g] << 24;
-                m[10] |= static_cast<int32_t>(mask2[g] << (8 * g));
-                m[2 + g] = wb;
-                m[6 + g] = static_cast<int32_t>(om);
-                wbmax = std::max(wbmax, wb);
-            }
-            const int len = kWinNS + wbmax + kWinOMax;  // even
-            if (base > INT32_MAX)
+    auto start_band = [&](int c) -> bool {
+        for (size_t k = 0; k < nrow; ++k) {
+            const int diff = rp[k][c] - r0[k][c];
+            if (diff < 0)
+                return false;  // DM list not monotone inside a row group
+            base[k] = theta[k] = std::max(0, diff - 1);
+        }
+        return true;
+    };
+    wp.band.push_back(0);
+    if (!start_band(0))
+        return false;
+    int kmax = 0;
+    for (int c = 1; c < nchans; ++c) {
+        bool split = false;
+        for (size_t k = 0; k < nrow && !split; ++k) {
+            const int diff = rp[k][c] - r0[k][c];
+            const int b = std::max(base[k], diff - 1);
+            nb[k] = b;
+            // infeasible offset, more than two shifts at once, or too many shifts in this band
+            if (b > diff || b - base[k] > 2 || b - theta[k] > kcap)
+                split = true;
+        }
+        if (split) {
+            if (c - wp.band.back() < 4)
+                return false;  // trials drift apart faster than the kernel can follow
+            wp.band.push_back(c);
+            if (!start_band(c))
                 return false;
-            m[0] = static_cast<int32_t>(base);
-            m[1] = len;
-            lmax = std::max(lmax, len);
-            maxbase = std::max(maxbase, base);
-        }
-        for (int r = 0; r < kWinDB; ++r) {
-            wp.kfinal[static_cast<size_t>(ty) * kWinDB + r] = kappa[r];
-            kmax = std::max(kmax, kappa[r]);
+        } else {
+            for (size_t k = 0; k < nrow; ++k) {
+                base[k] = nb[k];
+                kmax = std::max(kmax, base[k] - theta[k]);
+            }
         }
     }
-    const int H = (kWinNS - kmax) & ~1;
-    if (H < kWinNS / 2)  // more than half of the slots would be skew slack: not worth it
+    wp.band.push_back(nchans);
+    wp.nband = static_cast<int>(wp.band.size()) - 1;
+    if (wp.nband > 64)
+        return false;
+    const int H = W - kmax;
+    if (H < W / 2)
         return false;
     wp.H = H;
     wp.kmax = kmax;
+    wp.ntile_dm = ntile;
+
+    // ---- pass 2: metadata ---------------------------------------------------------------------------
+    wp.meta.assign(static_cast<size_t>(ntile) * nchans * kWinMetaWords, 0);
+    wp.kfinal.assign(static_cast<size_t>(ntile) * wp.nband * RB, 0);
+    wp.theta.assign(static_cast<size_t>(ntile) * wp.nband * RB, 0);
+    int lmax = 0, theta_max = 0;
+    int64_t maxbase = 0;
+    std::vector<int> bs(RB), th(RB);
+    for (int ty = 0; ty < ntile; ++ty) {
+        const size_t k0 = static_cast<size_t>(ty) * RB;
+        for (int b = 0; b < wp.nband; ++b) {
+            for (int c = wp.band[b]; c < wp.band[b + 1]; ++c) {
+                int32_t* m = wp.meta.data() + (static_cast<size_t>(ty) * nchans + c) * kWinMetaWords;
+                int64_t lo = INT64_MAX, hi = 0;
+                for (int g = 0; g < G; ++g) {
+                    const int64_t om = r0[k0 + g * kWinD][c];
+                    lo = std::min(lo, om);
+                    hi = std::max(hi, om);
+                }
+                const int64_t segbase = lo & ~static_cast<int64_t>(1);
+                if (segbase > INT32_MAX)
+                    return false;
+                int len = static_cast<int>(hi - segbase) + (geom.NT - 1) * H + W + 1;
+                len = (len + 1) & ~1;
+                m[0] = static_cast<int32_t>(segbase);
+                m[1] = len;
+                lmax = std::max(lmax, len);
+                maxbase = std::max(maxbase, segbase);
+                for (int g = 0; g < G; ++g) {
+                    const int64_t wb = r0[k0 + g * kWinD][c] - segbase;
+                    if (wb + (geom.NT - 1) * H >= (1 << kWinWbBits))
+                        return false;
+                    unsigned word = static_cast<unsigned>(wb) << 21;
+                    for (int j = 1; j < kWinD; ++j) {
+                        const int r = g * kWinD + j;
+                        const int diff = rp[k0 + r][c] - r0[k0 + r][c];
+                        if (c == wp.band[b])
+                            bs[r] = th[r] = std::max(0, diff - 1);
+                        const int nbase = std::max(bs[r], diff - 1);
+                        const int ns = nbase - bs[r], o = diff - nbase;
+                        if (o < 0 || o > 1 || ns > 2)
+                            return false;  // cannot happen after pass 1
+                        bs[r] = nbase;
+                        if (o)
+                            word |= 1u << (j - 1);
+                        if (ns >= 1)
+                            word |= 1u << (7 + j - 1);
+                        if (ns >= 2)
+                            word |= 1u << (14 + j - 1);
+                    }
+                    m[2 + g] = static_cast<int32_t>(word);
+                }
+            }
+            for (int r = 0; r < RB; ++r) {
+                const size_t k = (static_cast<size_t>(ty) * wp.nband + b) * RB + r;
+                const bool ref = r % kWinD == 0;
+                wp.kfinal[k] = ref ? 0 : bs[r] - th[r];
+                wp.theta[k] = ref ? 0 : th[r];
+                theta_max = std::max(theta_max, wp.theta[k]);
+            }
+        }
+    }
     wp.lmax = lmax;
     wp.maxbase = maxbase;
+    wp.theta_max = theta_max;
     wp.ok = true;
     return true;
 }
 
+int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out)
+{
+    const int64_t stride = 2LL * wp.geom.NT * wp.H;
+    return (n_out - 1 + wp.theta_max) / stride + 1;
+}
+
 int64_t window_pair_stride(const WindowPlan& wp, int64_t n_out)
 {
-    const int64_t ntile_t = (n_out + 2 * wp.H - 1) / (2 * wp.H);
-    int64_t n = ntile_t * 2 * wp.H + wp.maxbase + wp.lmax;
+    const int64_t n = window_ntile_t(wp, n_out) * 2 * wp.geom.NT * wp.H + wp.maxbase + wp.lmax + 2;
     return (n + 1) & ~static_cast<int64_t>(1);
 }
 
