@@ -123,12 +123,23 @@ template <int T> __device__ __forceinline__ void load_window(u64 (&w)[T + 1], co
         w[k] = q[k];
 }
 
-__device__ __forceinline__ void put(float* p, float v, bool first) { *p = first ? v : *p + v; }
+// band 0 stores; later bands add with a fire-and-forget reduction (one per cell and launch, launches
+// are stream-ordered, so the fp32 result does not depend on scheduling)
+__device__ __forceinline__ void put(float* p, float v, bool first)
+{
+    if (first)
+        *p = v;
+    else
+        asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+}
 // int32 output: the fp32 partial sums are exact integers (nchans * 255 < 2^24)
 __device__ __forceinline__ void put(int32_t* p, float v, bool first)
 {
     const int iv = __float2int_rn(v);
-    *p = first ? iv : *p + iv;
+    if (first)
+        *p = iv;
+    else
+        asm volatile("red.global.add.s32 [%0], %1;" ::"l"(p), "r"(iv) : "memory");
 }
 
 // smem layout: [nslot] full barriers | [nslot] empty barriers | transpose scratch [NCW][W] u64 | slots
@@ -166,23 +177,44 @@ __global__ void __launch_bounds__(G * NT * 32, 1)
     const float2* prow = static_cast<const float2*>(a.pairs) +
                          (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
     const int64_t pair_stride = a.pair_stride;
-    auto produce = [&](int i) {
-        const int s = i & (nslot - 1), lap = i >> nslot_log2;
-        if (lap > 0)
-            mbar_wait(bar_empty + 8u * s, (lap - 1) & 1);
-        const int32_t* m = meta + static_cast<int64_t>(i) * kWinMetaWords;
-        const int base = __ldg(m), len = __ldg(m + 1);
-        const unsigned dst = smem_u32(slots + static_cast<size_t>(s) * slot_bytes);
-        const unsigned fb = bar_full + 8u * s;
-        mbar_expect_tx(fb, kSlotHdr + len * 8);
-        bulk_g2s(dst, m, kSlotHdr, fb);
-        bulk_g2s(dst + kSlotHdr, prow + static_cast<int64_t>(i) * pair_stride + base, len * 8, fb);
+    // warp 0 keeps (base, len) of 32 channels in registers (lane L: channel 32*pq + L), loaded one
+    // batch ahead of use so that the staging thread never waits for a global load
+    int pb = 0, pl = 0, pbn = 0, pln = 0;
+    auto fetch_meta = [&](int q, int& b_, int& l_) {
+        const int k = q * 32 + lane;
+        if (k < nch) {
+            b_ = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords);
+            l_ = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords + 1);
+        }
+    };
+    auto produce = [&](int i) {  // called by all lanes of warp 0
+        if ((i & 31) == 0 && i > 0) {
+            pb = pbn;
+            pl = pln;
+        }
+        if ((i & 31) == 0)
+            fetch_meta((i >> 5) + 1, pbn, pln);
+        const int base = __shfl_sync(0xffffffffu, pb, i & 31), len = __shfl_sync(0xffffffffu, pl, i & 31);
+        if (lane == 0) {
+            const int s = i & (nslot - 1), lap = i >> nslot_log2;
+            if (lap > 0)
+                mbar_wait(bar_empty + 8u * s, (lap - 1) & 1);
+            const int32_t* m = meta + static_cast<int64_t>(i) * kWinMetaWords;
+            const unsigned dst = smem_u32(slots + static_cast<size_t>(s) * slot_bytes);
+            const unsigned fb = bar_full + 8u * s;
+            mbar_expect_tx(fb, kSlotHdr + len * 8);
+            bulk_g2s(dst, m, kSlotHdr, fb);
+            bulk_g2s(dst + kSlotHdr, prow + static_cast<int64_t>(i) * pair_stride + base, len * 8, fb);
+        }
+        __syncwarp();
     };
     const int lead = nslot - 4;
-    const bool producer = tid == 0;
-    if (producer)
+    const bool producer = warp == 0;
+    if (producer) {
+        fetch_meta(0, pb, pl);
         for (int i = 0; i < lead && i < nch; ++i)
             produce(i);
+    }
 
     // ---- consumers ------------------------------------------------------------------------------------
     const int g = warp / NT, wt = warp % NT;
