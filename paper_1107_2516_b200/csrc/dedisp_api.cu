@@ -88,7 +88,8 @@ struct dedisp_plan {
     // register-window kernel (brute-force plans): host plan, device tables, pair scratch
     WindowPlan win;
     bool win_fits = false;
-    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr, *d_win_theta = nullptr;
+    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr, *d_win_theta = nullptr, *d_win_hdr = nullptr;
+    void* d_win_zeros = nullptr;
     DevBuf pairs;
 };
 
@@ -131,6 +132,14 @@ dedisp_status upload(dedisp_plan* p)
                 e = up(&p->d_win_kfinal, p->win.kfinal);
             if (e == cudaSuccess)
                 e = up(&p->d_win_theta, p->win.theta);
+            if (e == cudaSuccess)
+                e = up(&p->d_win_hdr, p->win.hdr);
+            if (e == cudaSuccess) {
+                const size_t zb = static_cast<size_t>(p->win.lmax + 16) * 8;
+                e = cudaMalloc(&p->d_win_zeros, zb);
+                if (e == cudaSuccess)
+                    e = cudaMemset(p->d_win_zeros, 0, zb);
+            }
         }
     } else {
         e = up(&p->d_s1, p->s1);
@@ -176,6 +185,10 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.meta = plan->d_win_meta;
     a.kfinal = plan->d_win_kfinal;
     a.theta = plan->d_win_theta;
+    a.hdr = plan->d_win_hdr;
+    a.zeros = plan->d_win_zeros;
+    a.stage0 = plan->win.stage0.data();
+    a.stage_total = plan->win.stage0[plan->win.nband];
     a.nband = plan->win.nband;
     a.band = plan->win.band.data();
     a.geom = plan->win.geom;
@@ -389,6 +402,8 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaFree(p->d_win_meta);
         cudaFree(p->d_win_kfinal);
         cudaFree(p->d_win_theta);
+        cudaFree(p->d_win_hdr);
+        cudaFree(p->d_win_zeros);
     }
     p->pairs.release();
     p->scratch.release();

@@ -53,7 +53,9 @@ int launch_direct(const Problem& p, Elem in_t, const int spread[3], void* stream
 // (+ 1 producer warp); the channel loop is cut into bands, one launch per band.
 constexpr int kWinD = 8;            // DM rows per thread
 constexpr int kWinMetaWords = 16;   // per (DM tile, channel) metadata, 64 bytes
-constexpr int kWinWbBits = 11;      // window offset inside the staged segment, in pairs
+constexpr int kWinWbBits = 11;
+constexpr int kWinCh = 4;           // channels per pipeline stage (one mbarrier pair per stage)
+constexpr int kWinHdrWords = 32;    // per (DM tile, stage) header: [row group][kWinCh] words, 128 bytes      // window offset inside the staged segment, in pairs
 
 struct WindowGeom {
     int T = 0;   // slots per lane and row (odd: conflict-free LDS.64)
@@ -78,6 +80,8 @@ struct WindowPlan {
     // and, per row group, jitter bits (rows 1..7) | shift mask << 7 | 2nd shift mask << 14 |
     // window offset << 21
     std::vector<int32_t> meta;
+    std::vector<int32_t> stage0;  // [nband + 1] first stage of every band in hdr
+    std::vector<int32_t> hdr;     // [tile][stage0[nband]][kWinHdrWords]
     std::vector<int32_t> kfinal;  // [tile][band][rows] row shifts of every row at the band's end
     std::vector<int32_t> theta;   // [tile][band][rows] band skew of every row
 };
@@ -93,8 +97,11 @@ struct WindowArgs {
     const int32_t* kfinal;
     const int32_t* theta;
     int64_t in_stride, out_stride, pair_stride, in_len, n_out;
-    int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t, nband;
-    const int32_t* band;  // HOST pointer, [nband + 1]
+    int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t, nband, stage_total;
+    const int32_t* band;    // HOST pointer, [nband + 1]
+    const int32_t* stage0;  // HOST pointer, [nband + 1]
+    const int32_t* hdr;     // device copy of WindowPlan::hdr
+    const void* zeros;      // device, >= lmax pairs of zeros (segments of the padding channels)
     WindowGeom geom;
 };
 bool window_fits_smem(const WindowPlan& wp);

@@ -68,6 +68,15 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive_lane0(unsigned bar, int lane)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.eq.s32 p, %1, 0;\n"
+        "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n"
+        "}\n" ::"r"(bar), "r"(lane) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
     asm volatile(
@@ -98,19 +107,21 @@ __device__ __forceinline__ u64 add2(u64 a, u64 b)
 // ------------------------------------------------------------------------------------------------
 // 2. window kernel
 // ------------------------------------------------------------------------------------------------
-constexpr int kSlotHdr = kWinMetaWords * 4;  // bytes of metadata in front of a staged segment
 
-// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one
+// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one.
+// The moves are written as x + (-0.0) (exact for every x) instead of register copies: ptxas
+// would otherwise coalesce the copies by rotating the accumulator registers inside the hot loop.
 template <int T> __device__ __forceinline__ void shift_rows(u64 (&acc)[kWinD][T], unsigned mask, int lane)
 {
+    const u64 nz = 0x8000000080000000ull;
 #pragma unroll
     for (int j = 1; j < kWinD; ++j) {
         if (mask & (1u << (j - 1))) {
             const u64 carry = __shfl_up_sync(0xffffffffu, acc[j][T - 1], 1);
 #pragma unroll
             for (int i = T - 1; i > 0; --i)
-                acc[j][i] = acc[j][i - 1];
-            acc[j][0] = lane ? carry : 0ull;
+                asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(acc[j][i]) : "l"(acc[j][i - 1]), "l"(nz));
+            asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(acc[j][0]) : "l"(lane ? carry : 0ull), "l"(nz));
         }
     }
 }
@@ -142,27 +153,32 @@ __device__ __forceinline__ void put(int32_t* p, float v, bool first)
         asm volatile("red.global.add.s32 [%0], %1;" ::"l"(p), "r"(iv) : "memory");
 }
 
-// smem layout: [nslot] full barriers | [nslot] empty barriers | transpose scratch [NCW][W] u64 | slots
+// smem layout: [nst] full barriers | [nst] empty barriers | transpose scratch [NCW][W] u64 |
+//              nst stages of { 128-byte header, kWinCh channel slots }
 template <int T, int G, int NT, typename OutT>
-__global__ void __launch_bounds__(G * NT * 32, 1)
-    window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int nslot_log2,
-                  const int slot_bytes)
+__global__ void __launch_bounds__((G * NT + 4) * 32, 1)
+    window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0,
+                  const int nst, const int slot_bytes)
 {
     constexpr int W = 32 * T, NCW = G * NT, RB = kWinD * G;
+    // registers per consumer thread once the producer warp group has released its share
+    constexpr int kPool = (65536 - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
+    constexpr int kConsRegs = kPool > 240 ? 240 : kPool;
+    static_assert(NCW % 4 == 0, "setmaxnreg works on groups of four warps");
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ty = blockIdx.x, beam = blockIdx.z;
     const int64_t T0 = static_cast<int64_t>(blockIdx.y) * 2 * NT * a.H;
-    const int nslot = 1 << nslot_log2;
 
     const unsigned bar_full = smem_u32(smem);
-    const unsigned bar_empty = bar_full + 8u * nslot;
-    const int tr_off = (16 * nslot + 127) & ~127;
-    const int slots_off = (tr_off + NCW * W * 8 + 127) & ~127;
-    unsigned char* slots = smem + slots_off;
+    const unsigned bar_empty = bar_full + 8u * nst;
+    const int tr_off = (16 * nst + 127) & ~127;
+    const int stages_off = (tr_off + NCW * W * 8 + 127) & ~127;
+    const int stage_bytes = kWinHdrWords * 4 + kWinCh * slot_bytes;
+    unsigned char* stages = smem + stages_off;
 
     if (tid == 0) {
-        for (int s = 0; s < nslot; ++s) {
+        for (int s = 0; s < nst; ++s) {
             mbar_init(bar_full + 8u * s, 1);
             mbar_init(bar_empty + 8u * s, NCW);
         }
@@ -171,50 +187,69 @@ __global__ void __launch_bounds__(G * NT * 32, 1)
     __syncthreads();
 
     const int nch = c_end - c_begin;
-    const int32_t* meta = a.meta + (static_cast<int64_t>(ty) * a.nchans + c_begin) * kWinMetaWords;
+    const int nstage = (nch + kWinCh - 1) / kWinCh;  // the producer stages one more (all padding)
+    const int stage_total = a.stage_total;
 
-    // ---- producer duty (thread 0): stage channel i into slot i % nslot, kLead channels ahead ------------
-    const float2* prow = static_cast<const float2*>(a.pairs) +
-                         (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
-    const int64_t pair_stride = a.pair_stride;
-    // warp 0 keeps (base, len) of 32 channels in registers (lane L: channel 32*pq + L), loaded one
-    // batch ahead of use so that the staging thread never waits for a global load
-    int pb = 0, pl = 0, pbn = 0, pln = 0;
-    auto fetch_meta = [&](int q, int& b_, int& l_) {
-        const int k = q * 32 + lane;
-        if (k < nch) {
-            b_ = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords);
-            l_ = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords + 1);
+    if (warp >= NCW) {
+        // ---- producer warp group: gives its registers to the consumers; one thread stages kWinCh
+        // channels per barrier (padding channels and the extra last stage get zeros)
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (warp == NCW) {
+            const int32_t* meta = a.meta + (static_cast<int64_t>(ty) * a.nchans + c_begin) * kWinMetaWords;
+            const int32_t* hdr = a.hdr + (static_cast<int64_t>(ty) * stage_total + stage0) * kWinHdrWords;
+            const float2* prow = static_cast<const float2*>(a.pairs) +
+                                 (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
+            const int64_t pair_stride = a.pair_stride;
+            const int zlen = ((NT - 1) * a.H + W + 2 + 1) & ~1;  // pairs a padding channel must provide
+            int pb = 0, pl = 0;  // lane L: (base, len) of channel 32*q + L
+            int ring = 0, lap = 0;
+            for (int s = 0; s <= nstage; ++s) {
+                if ((s & 7) == 0) {  // 8 stages = 32 channels per metadata fetch
+                    const int k = s * kWinCh + lane;
+                    pb = 0;
+                    pl = -1;
+                    if (k < nch) {
+                        pb = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords);
+                        pl = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords + 1);
+                    }
+                }
+                int base[kWinCh], len[kWinCh];
+#pragma unroll
+                for (int ch = 0; ch < kWinCh; ++ch) {
+                    base[ch] = __shfl_sync(0xffffffffu, pb, ((s & 7) * kWinCh + ch) & 31);
+                    len[ch] = __shfl_sync(0xffffffffu, pl, ((s & 7) * kWinCh + ch) & 31);
+                }
+                if (lane == 0) {
+                    if (lap > 0)
+                        mbar_wait(bar_empty + 8u * ring, (lap - 1) & 1);
+                    const unsigned dst = smem_u32(stages) + ring * stage_bytes;
+                    const unsigned fb = bar_full + 8u * ring;
+                    unsigned bytes = kWinHdrWords * 4;
+#pragma unroll
+                    for (int ch = 0; ch < kWinCh; ++ch)
+                        bytes += (len[ch] < 0 ? zlen : len[ch]) * 8;
+                    mbar_expect_tx(fb, bytes);
+                    bulk_g2s(dst, hdr + static_cast<int64_t>(s) * kWinHdrWords, kWinHdrWords * 4, fb);
+#pragma unroll
+                    for (int ch = 0; ch < kWinCh; ++ch) {
+                        const unsigned d = dst + kWinHdrWords * 4 + ch * slot_bytes;
+                        if (len[ch] < 0)
+                            bulk_g2s(d, a.zeros, zlen * 8, fb);
+                        else
+                            bulk_g2s(d, prow + static_cast<int64_t>(s * kWinCh + ch) * pair_stride + base[ch],
+                                     len[ch] * 8, fb);
+                    }
+                }
+                __syncwarp();
+                if (++ring == nst) {
+                    ring = 0;
+                    ++lap;
+                }
+            }
         }
-    };
-    auto produce = [&](int i) {  // called by all lanes of warp 0
-        if ((i & 31) == 0 && i > 0) {
-            pb = pbn;
-            pl = pln;
-        }
-        if ((i & 31) == 0)
-            fetch_meta((i >> 5) + 1, pbn, pln);
-        const int base = __shfl_sync(0xffffffffu, pb, i & 31), len = __shfl_sync(0xffffffffu, pl, i & 31);
-        if (lane == 0) {
-            const int s = i & (nslot - 1), lap = i >> nslot_log2;
-            if (lap > 0)
-                mbar_wait(bar_empty + 8u * s, (lap - 1) & 1);
-            const int32_t* m = meta + static_cast<int64_t>(i) * kWinMetaWords;
-            const unsigned dst = smem_u32(slots + static_cast<size_t>(s) * slot_bytes);
-            const unsigned fb = bar_full + 8u * s;
-            mbar_expect_tx(fb, kSlotHdr + len * 8);
-            bulk_g2s(dst, m, kSlotHdr, fb);
-            bulk_g2s(dst + kSlotHdr, prow + static_cast<int64_t>(i) * pair_stride + base, len * 8, fb);
-        }
-        __syncwarp();
-    };
-    const int lead = nslot - 4;
-    const bool producer = warp == 0;
-    if (producer) {
-        fetch_meta(0, pb, pl);
-        for (int i = 0; i < lead && i < nch; ++i)
-            produce(i);
+        return;
     }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kConsRegs));
 
     // ---- consumers ------------------------------------------------------------------------------------
     const int g = warp / NT, wt = warp % NT;
@@ -225,53 +260,56 @@ __global__ void __launch_bounds__(G * NT * 32, 1)
         for (int i = 0; i < T; ++i)
             acc[j][i] = 0ull;
 
-    const int lane_off = kSlotHdr + (wt * a.H + lane * T) * 8;  // bytes from the slot start
-    auto slot_ptr = [&](int i) { return slots + static_cast<size_t>(i & (nslot - 1)) * slot_bytes; };
-    auto wait_full = [&](int i) { mbar_wait(bar_full + 8u * (i & (nslot - 1)), (i >> nslot_log2) & 1); };
-    auto slot_word = [&](int i) { return reinterpret_cast<const unsigned*>(slot_ptr(i))[2 + g]; };
-
-    // software pipeline: channel i is added from w/m while the window of i+1 and the metadata of
-    // i+2 are on their way
-    u64 wa[T + 1], wb[T + 1];
-    unsigned m = 0, mn = 0, mnn = 0;
-    wait_full(0);
-    m = slot_word(0);
-    if (nch > 1) {
-        wait_full(1);
-        mn = slot_word(1);
-    }
-    load_window<T>(wa, slot_ptr(0) + lane_off + (m >> 21) * 8);
-
-    auto step = [&](int i, u64(&w)[T + 1], u64(&wn)[T + 1]) {
-        if (producer && i + lead < nch)
-            produce(i + lead);
-        if (i + 1 < nch)
-            load_window<T>(wn, slot_ptr(i + 1) + lane_off + (mn >> 21) * 8);
-        if (i + 2 < nch) {
-            wait_full(i + 2);
-            mnn = slot_word(i + 2);
-        }
+    // per stage: wait for the NEXT stage and read its four metadata words with one LDS.128, then
+    // add the four channels of this stage; the window of channel k+1 is loaded while channel k is
+    // added (wa / wb alternate).
+    const unsigned lane_off = kWinHdrWords * 4 + (wt * a.H + lane * T) * 8;  // bytes from the stage start
+    auto channel = [&](u64(&w)[T + 1], unsigned m) {
         const unsigned sm = (m >> 7) & 0x3fffu;
         if (sm) {
             shift_rows<T>(acc, sm & 127u, lane);
             if (sm >> 7)
                 shift_rows<T>(acc, sm >> 7, lane);
         }
+#ifndef DEDISP_EXP_NOMATH
 #pragma unroll
         for (int k = 0; k < T; ++k)
             acc[0][k] = add2(acc[0][k], w[k]);
         rows7(acc, w, m);
-        __syncwarp();
-        if (lane == 0)
-            mbar_arrive(bar_empty + 8u * (i & (nslot - 1)));
-        m = mn;
-        mn = mnn;
+#else
+        acc[0][0] = add2(acc[0][0], w[0] ^ w[T]);
+#endif
     };
+    u64 wa[T + 1], wb[T + 1];
+    int ring = 0, par = 0;
+    mbar_wait(bar_full, 0);
+    const unsigned char* sp = stages;
+    uint4 mw = *reinterpret_cast<const uint4*>(sp + 16 * g);
+    load_window<T>(wa, sp + lane_off + (mw.x >> 21) * 8);
 #pragma unroll 1
-    for (int i = 0; i < nch; i += 2) {
-        step(i, wa, wb);
-        if (i + 1 < nch)
-            step(i + 1, wb, wa);
+    for (int s = 0; s < nstage; ++s) {
+        int nring = ring + 1, npar = par;
+        if (nring == nst) {
+            nring = 0;
+            npar ^= 1;
+        }
+        mbar_wait(bar_full + 8u * nring, npar);
+        const unsigned char* spn = stages + nring * stage_bytes;
+        const uint4 mn = *reinterpret_cast<const uint4*>(spn + 16 * g);
+        load_window<T>(wb, sp + slot_bytes + lane_off + (mw.y >> 21) * 8);
+        channel(wa, mw.x);
+        load_window<T>(wa, sp + 2 * slot_bytes + lane_off + (mw.z >> 21) * 8);
+        channel(wb, mw.y);
+        load_window<T>(wb, sp + 3 * slot_bytes + lane_off + (mw.w >> 21) * 8);
+        channel(wa, mw.z);
+        load_window<T>(wa, spn + lane_off + (mn.x >> 21) * 8);
+        channel(wb, mw.w);
+        __syncwarp();
+        mbar_arrive_lane0(bar_empty + 8u * ring, lane);
+        sp = spn;
+        mw = mn;
+        ring = nring;
+        par = npar;
     }
 
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
@@ -307,43 +345,45 @@ __global__ void __launch_bounds__(G * NT * 32, 1)
 // ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
-static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes, int* nslot_log2)
+// number of pipeline stages that fit into shared memory (0: the kernel cannot run)
+static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes)
 {
-    const int sb = (kSlotHdr + lmax * 8 + 127) & ~127;
+    const int sb = (lmax * 8 + 127) & ~127;
     const int fixed = 256 + g.G * g.NT * g.W() * 8 + 256;
     const int budget = 227 * 1024 - fixed;
-    int lg = 4;  // at most 16 slots
-    while (lg > 3 && (sb << lg) > budget)
-        --lg;
+    const int stage_bytes = kWinHdrWords * 4 + kWinCh * sb;
+    int nst = budget / stage_bytes;
+    if (nst > 8)
+        nst = 8;
     *slot_bytes = sb;
-    *nslot_log2 = lg;
-    return (sb << lg) <= budget ? (1 << lg) : 0;
+    return nst >= 3 ? nst : 0;
 }
 
 bool window_fits_smem(const WindowPlan& wp)
 {
-    int sb, lg;
-    return wp.ok && window_ring(wp.geom, wp.lmax, &sb, &lg) >= 8;
+    int sb;
+    return wp.ok && window_ring(wp.geom, wp.lmax, &sb) > 0;
 }
 
 template <int T, int G, int NT, typename OutT>
 static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
 {
-    int slot_bytes = 0, lg = 0;
-    const int nslot = window_ring(a.geom, a.lmax, &slot_bytes, &lg);
-    if (nslot < 8)
+    int slot_bytes = 0;
+    const int nst = window_ring(a.geom, a.lmax, &slot_bytes);
+    if (nst == 0)
         return static_cast<int>(cudaErrorInvalidConfiguration);
-    const int tr_off = (16 * nslot + 127) & ~127;
-    const int slots_off = (tr_off + G * NT * 32 * T * 8 + 127) & ~127;
-    const size_t smem = static_cast<size_t>(slots_off) + static_cast<size_t>(nslot) * slot_bytes;
+    const int tr_off = (16 * nst + 127) & ~127;
+    const int stages_off = (tr_off + G * NT * 32 * T * 8 + 127) & ~127;
+    const size_t smem = static_cast<size_t>(stages_off) +
+                        static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
     cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
         return static_cast<int>(e);
     dim3 grid(a.ntile_dm, a.ntile_t, a.nbeams);
     for (int b = 0; b < a.nband; ++b) {
-        window_kernel<T, G, NT, OutT><<<grid, G * NT * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b, lg,
-                                                                              slot_bytes);
+        window_kernel<T, G, NT, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b,
+                                                                              a.stage0[b], nst, slot_bytes);
         ++*launches;
         e = cudaGetLastError();
         if (e != cudaSuccess)
@@ -357,8 +397,10 @@ template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_
     const WindowGeom& g = a.geom;
     if (g.T == 9 && g.G == 8 && g.NT == 1)
         return launch_bands<9, 8, 1, OutT>(a, st, launches);
-    if (g.T == 5 && g.G == 8 && g.NT == 2)
-        return launch_bands<5, 8, 2, OutT>(a, st, launches);
+    if (g.T == 7 && g.G == 6 && g.NT == 2)
+        return launch_bands<7, 6, 2, OutT>(a, st, launches);
+    if (g.T == 5 && g.G == 6 && g.NT == 2)
+        return launch_bands<5, 6, 2, OutT>(a, st, launches);
     if (g.T == 7 && g.G == 4 && g.NT == 3)
         return launch_bands<7, 4, 3, OutT>(a, st, launches);
     return static_cast<int>(cudaErrorInvalidConfiguration);

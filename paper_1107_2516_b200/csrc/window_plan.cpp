@@ -16,6 +16,8 @@
 //     partial sums are added to the output by a later launch (kernels_window.cu).
 // Everything the kernel needs per (DM tile, channel) is precomputed into WindowPlan::meta.
 #include <algorithm>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "dedisp_internal.h"
@@ -28,6 +30,15 @@ WindowGeom window_default_geom()
     g.T = 9;
     g.G = 8;
     g.NT = 1;
+    // development override: DEDISP_WINDOW_GEOM="T,G,NT" (one of the instantiated geometries)
+    if (const char* e = std::getenv("DEDISP_WINDOW_GEOM")) {
+        int t = 0, gg = 0, nt = 0;
+        if (std::sscanf(e, "%d,%d,%d", &t, &gg, &nt) == 3) {
+            g.T = t;
+            g.G = gg;
+            g.NT = nt;
+        }
+    }
     return g;
 }
 
@@ -173,6 +184,24 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
             }
         }
     }
+    // ---- stage headers: the kernel consumes kWinCh channels per barrier; the words of those channels
+    // are regrouped per row group (hdr[g * kWinCh + ch]) so that a warp reads them with one LDS.128.
+    // Channels past the band's end and one extra stage per band stay zero (the kernel stages a
+    // zero segment for them).
+    wp.stage0.assign(wp.nband + 1, 0);
+    for (int b = 0; b < wp.nband; ++b)
+        wp.stage0[b + 1] = wp.stage0[b] + (wp.band[b + 1] - wp.band[b] + kWinCh - 1) / kWinCh + 1;
+    const int nst = wp.stage0[wp.nband];
+    wp.hdr.assign(static_cast<size_t>(ntile) * nst * kWinHdrWords, 0);
+    for (int ty = 0; ty < ntile; ++ty)
+        for (int b = 0; b < wp.nband; ++b)
+            for (int c = wp.band[b]; c < wp.band[b + 1]; ++c) {
+                const int s = wp.stage0[b] + (c - wp.band[b]) / kWinCh, ch = (c - wp.band[b]) % kWinCh;
+                const int32_t* m = wp.meta.data() + (static_cast<size_t>(ty) * nchans + c) * kWinMetaWords;
+                int32_t* h = wp.hdr.data() + (static_cast<size_t>(ty) * nst + s) * kWinHdrWords;
+                for (int g = 0; g < G; ++g)
+                    h[g * kWinCh + ch] = m[2 + g];
+            }
     wp.lmax = lmax;
     wp.maxbase = maxbase;
     wp.theta_max = theta_max;
