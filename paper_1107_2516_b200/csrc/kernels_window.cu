@@ -285,6 +285,10 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     mbar_wait(bar_full, 0);
     const unsigned char* sp = stages;
     uint4 mw = *reinterpret_cast<const uint4*>(sp + 16 * g);
+    mw.x = __reduce_or_sync(0xffffffffu, mw.x);
+    mw.y = __reduce_or_sync(0xffffffffu, mw.y);
+    mw.z = __reduce_or_sync(0xffffffffu, mw.z);
+    mw.w = __reduce_or_sync(0xffffffffu, mw.w);
     load_window<T>(wa, sp + lane_off + (mw.x >> 21) * 8);
 #pragma unroll 1
     for (int s = 0; s < nstage; ++s) {
@@ -295,7 +299,13 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
         }
         mbar_wait(bar_full + 8u * nring, npar);
         const unsigned char* spn = stages + nring * stage_bytes;
-        const uint4 mn = *reinterpret_cast<const uint4*>(spn + 16 * g);
+        uint4 mn = *reinterpret_cast<const uint4*>(spn + 16 * g);
+        // the words are the same in every lane; the reduction tells ptxas so (uniform registers), which
+        // keeps convergence barriers out of the row branches
+        mn.x = __reduce_or_sync(0xffffffffu, mn.x);
+        mn.y = __reduce_or_sync(0xffffffffu, mn.y);
+        mn.z = __reduce_or_sync(0xffffffffu, mn.z);
+        mn.w = __reduce_or_sync(0xffffffffu, mn.w);
         load_window<T>(wb, sp + slot_bytes + lane_off + (mw.y >> 21) * 8);
         channel(wa, mw.x);
         load_window<T>(wa, sp + 2 * slot_bytes + lane_off + (mw.z >> 21) * 8);
