@@ -108,20 +108,14 @@ __device__ __forceinline__ u64 add2(u64 a, u64 b)
 // 2. window kernel
 // ------------------------------------------------------------------------------------------------
 
-// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one.
-// The moves are written as x + (-0.0) (exact for every x) instead of register copies: ptxas
-// would otherwise coalesce the copies by rotating the accumulator registers inside the hot loop.
+// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one
 template <int T> __device__ __forceinline__ void shift_rows(u64 (&acc)[kWinD][T], unsigned mask, int lane)
 {
-    const u64 nz = 0x8000000080000000ull;
 #pragma unroll
     for (int j = 1; j < kWinD; ++j) {
         if (mask & (1u << (j - 1))) {
             const u64 carry = __shfl_up_sync(0xffffffffu, acc[j][T - 1], 1);
-#pragma unroll
-            for (int i = T - 1; i > 0; --i)
-                asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(acc[j][i]) : "l"(acc[j][i - 1]), "l"(nz));
-            asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(acc[j][0]) : "l"(lane ? carry : 0ull), "l"(nz));
+            shift_row(acc[j], lane ? carry : 0ull);
         }
     }
 }
@@ -280,46 +274,48 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
         acc[0][0] = add2(acc[0][0], w[0] ^ w[T]);
 #endif
     };
-    u64 wa[T + 1], wb[T + 1];
-    int ring = 0, par = 0;
+    // One channel per loop iteration (a single copy of the add block: ptxas permutes the
+    // accumulator registers between copies otherwise).  While channel c is added, the window of
+    // c+1 is loaded into wn and the metadata word of c+2 is fetched; the cursor (ring2, par2,
+    // ch2, st2) points at channel c+2.
+    u64 w[T + 1], wn[T + 1];
+    const unsigned hdr_off = 16 * g;
     mbar_wait(bar_full, 0);
-    const unsigned char* sp = stages;
-    uint4 mw = *reinterpret_cast<const uint4*>(sp + 16 * g);
-    mw.x = __reduce_or_sync(0xffffffffu, mw.x);
-    mw.y = __reduce_or_sync(0xffffffffu, mw.y);
-    mw.z = __reduce_or_sync(0xffffffffu, mw.z);
-    mw.w = __reduce_or_sync(0xffffffffu, mw.w);
-    load_window<T>(wa, sp + lane_off + (mw.x >> 21) * 8);
+    unsigned m0 = __reduce_or_sync(0xffffffffu, *reinterpret_cast<const unsigned*>(stages + hdr_off));
+    unsigned m1 = __reduce_or_sync(0xffffffffu, *reinterpret_cast<const unsigned*>(stages + hdr_off + 4));
+    load_window<T>(w, stages + lane_off + (m0 >> 21) * 8);
+    const unsigned char* st2 = stages;          // stage of channel c+2
+    const unsigned char* p1 = stages + slot_bytes;  // slot of channel c+1 (without the header offset)
+    int ring2 = 0, par2 = 0, ch2 = 2, ring0 = 0;
+    const int ntot = nstage * kWinCh;
 #pragma unroll 1
-    for (int s = 0; s < nstage; ++s) {
-        int nring = ring + 1, npar = par;
-        if (nring == nst) {
-            nring = 0;
-            npar ^= 1;
+    for (int c = 0; c < ntot; ++c) {
+        load_window<T>(wn, p1 + lane_off + (m1 >> 21) * 8);
+        if (ch2 == 0)
+            mbar_wait(bar_full + 8u * ring2, par2);
+        const unsigned m2 =
+            __reduce_or_sync(0xffffffffu, *reinterpret_cast<const unsigned*>(st2 + hdr_off + 4 * ch2));
+        p1 = st2 + ch2 * slot_bytes;
+        channel(w, m0);
+        if ((c & (kWinCh - 1)) == kWinCh - 1) {
+            __syncwarp();
+            mbar_arrive_lane0(bar_empty + 8u * ring0, lane);
+            if (++ring0 == nst)
+                ring0 = 0;
         }
-        mbar_wait(bar_full + 8u * nring, npar);
-        const unsigned char* spn = stages + nring * stage_bytes;
-        uint4 mn = *reinterpret_cast<const uint4*>(spn + 16 * g);
-        // the words are the same in every lane; the reduction tells ptxas so (uniform registers), which
-        // keeps convergence barriers out of the row branches
-        mn.x = __reduce_or_sync(0xffffffffu, mn.x);
-        mn.y = __reduce_or_sync(0xffffffffu, mn.y);
-        mn.z = __reduce_or_sync(0xffffffffu, mn.z);
-        mn.w = __reduce_or_sync(0xffffffffu, mn.w);
-        load_window<T>(wb, sp + slot_bytes + lane_off + (mw.y >> 21) * 8);
-        channel(wa, mw.x);
-        load_window<T>(wa, sp + 2 * slot_bytes + lane_off + (mw.z >> 21) * 8);
-        channel(wb, mw.y);
-        load_window<T>(wb, sp + 3 * slot_bytes + lane_off + (mw.w >> 21) * 8);
-        channel(wa, mw.z);
-        load_window<T>(wa, spn + lane_off + (mn.x >> 21) * 8);
-        channel(wb, mw.w);
-        __syncwarp();
-        mbar_arrive_lane0(bar_empty + 8u * ring, lane);
-        sp = spn;
-        mw = mn;
-        ring = nring;
-        par = npar;
+        if (++ch2 == kWinCh) {
+            ch2 = 0;
+            if (++ring2 == nst) {
+                ring2 = 0;
+                par2 ^= 1;
+            }
+            st2 = stages + ring2 * stage_bytes;
+        }
+#pragma unroll
+        for (int k = 0; k <= T; ++k)
+            w[k] = wn[k];
+        m0 = m1;
+        m1 = m2;
     }
 
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
