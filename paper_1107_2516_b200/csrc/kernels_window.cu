@@ -246,7 +246,12 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kConsRegs));
 
     // ---- consumers ------------------------------------------------------------------------------------
-    const int g = warp / NT, wt = warp % NT;
+    // the warp index through a reduction: ptxas then knows it (and every shared-memory word loaded
+    // from an address built from it) is warp-uniform, so the row branches become BRA.U
+    const int uwarp = __reduce_or_sync(0xffffffffu, warp);
+    const int g = uwarp / NT, wt = uwarp % NT;
+    int lane_pinned;  // volatile: not rematerialised (S2R) inside the channel loop
+    asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane_pinned));
     u64 acc[kWinD][T];
 #pragma unroll
     for (int j = 0; j < kWinD; ++j)
@@ -257,13 +262,13 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     // per stage: wait for the NEXT stage and read its four metadata words with one LDS.128, then
     // add the four channels of this stage; the window of channel k+1 is loaded while channel k is
     // added (wa / wb alternate).
-    const unsigned lane_off = kWinHdrWords * 4 + (wt * a.H + lane * T) * 8;  // bytes from the stage start
+    const unsigned lane_off = kWinHdrWords * 4 + (wt * a.H + lane_pinned * T) * 8;  // bytes from the slot start
     auto channel = [&](u64(&w)[T + 1], unsigned m) {
         const unsigned sm = (m >> 7) & 0x3fffu;
         if (sm) {
-            shift_rows<T>(acc, sm & 127u, lane);
+            shift_rows<T>(acc, sm & 127u, lane_pinned);
             if (sm >> 7)
-                shift_rows<T>(acc, sm >> 7, lane);
+                shift_rows<T>(acc, sm >> 7, lane_pinned);
         }
 #ifndef DEDISP_EXP_NOMATH
 #pragma unroll
@@ -281,8 +286,8 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     u64 w[T + 1], wn[T + 1];
     const unsigned hdr_off = 16 * g;
     mbar_wait(bar_full, 0);
-    unsigned m0 = __reduce_or_sync(0xffffffffu, *reinterpret_cast<const unsigned*>(stages + hdr_off));
-    unsigned m1 = __reduce_or_sync(0xffffffffu, *reinterpret_cast<const unsigned*>(stages + hdr_off + 4));
+    unsigned m0 = *reinterpret_cast<const unsigned*>(stages + hdr_off);
+    unsigned m1 = *reinterpret_cast<const unsigned*>(stages + hdr_off + 4);
     load_window<T>(w, stages + lane_off + (m0 >> 21) * 8);
     const unsigned char* st2 = stages;          // stage of channel c+2
     const unsigned char* p1 = stages + slot_bytes;  // slot of channel c+1 (without the header offset)
@@ -293,13 +298,12 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
         load_window<T>(wn, p1 + lane_off + (m1 >> 21) * 8);
         if (ch2 == 0)
             mbar_wait(bar_full + 8u * ring2, par2);
-        const unsigned m2 =
-            __reduce_or_sync(0xffffffffu, *reinterpret_cast<const unsigned*>(st2 + hdr_off + 4 * ch2));
+        const unsigned m2 = *reinterpret_cast<const unsigned*>(st2 + hdr_off + 4 * ch2);
         p1 = st2 + ch2 * slot_bytes;
         channel(w, m0);
         if ((c & (kWinCh - 1)) == kWinCh - 1) {
             __syncwarp();
-            mbar_arrive_lane0(bar_empty + 8u * ring0, lane);
+            mbar_arrive_lane0(bar_empty + 8u * ring0, lane_pinned);
             if (++ring0 == nst)
                 ring0 = 0;
         }
