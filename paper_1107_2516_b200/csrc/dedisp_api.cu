@@ -189,6 +189,7 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.zeros = plan->d_win_zeros;
     a.stage0 = plan->win.stage0.data();
     a.stage_total = plan->win.stage0[plan->win.nband];
+    a.theta_max = plan->win.theta_max;
     a.nband = plan->win.nband;
     a.band = plan->win.band.data();
     a.geom = plan->win.geom;

@@ -252,6 +252,10 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     const int g = uwarp / NT, wt = uwarp % NT;
     int lane_pinned;  // volatile: not rematerialised (S2R) inside the channel loop
     asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane_pinned));
+    // lanes 0..7 fetch the flush parameters of rows 0..7 now, long before they are needed
+    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
+    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
+    const int kf_lane = __ldg(kfp + (lane_pinned & 7)), th_lane = __ldg(thp + (lane_pinned & 7));
     u64 acc[kWinD][T];
 #pragma unroll
     for (int j = 0; j < kWinD; ++j)
@@ -325,28 +329,48 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
     u64* tr = reinterpret_cast<u64*>(smem + tr_off) + warp * W;
     const bool first = band == 0;
-    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
-    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
     OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
-    const int64_t hp = static_cast<int64_t>(NT) * a.H;
+    const int H = a.H;
+    const int64_t hp = static_cast<int64_t>(NT) * H;
+    const int64_t tw = T0 + wt * H;
+    // every sample of this warp's two output ranges inside [0, n_out): no bounds tests
+    const bool inside = tw - a.theta_max >= 0 && tw + hp + H <= a.n_out;
 #pragma unroll
     for (int j = 0; j < kWinD; ++j) {
         const int d = ty * RB + g * kWinD + j;
+        const int kf = __shfl_sync(0xffffffffu, kf_lane, j), th = __shfl_sync(0xffffffffu, th_lane, j);
         __syncwarp();
 #pragma unroll
         for (int i = 0; i < T; ++i)
-            tr[lane * T + i] = acc[j][i];
+            tr[lane_pinned * T + i] = acc[j][i];
         __syncwarp();
         if (d < a.ndm) {
-            const int kf = __ldg(kfp + j), th = __ldg(thp + j);
-            OutT* o = out + static_cast<int64_t>(d) * a.out_stride;
-            for (int q = lane; q < a.H; q += 32) {
-                const u64 v = tr[q + kf];
-                const int64_t t = T0 + wt * a.H + q - th;
-                if (t >= 0 && t < a.n_out)
-                    put(o + t, __uint_as_float(static_cast<unsigned>(v)), first);
-                if (t + hp >= 0 && t + hp < a.n_out)
-                    put(o + t + hp, __uint_as_float(static_cast<unsigned>(v >> 32)), first);
+            OutT* o = out + static_cast<int64_t>(d) * a.out_stride + (tw - th);
+            u64 v[T];
+#pragma unroll
+            for (int k = 0; k < T; ++k) {
+                const int q = lane_pinned + 32 * k;
+                v[k] = q < H ? tr[q + kf] : 0ull;
+            }
+            if (inside) {
+#pragma unroll
+                for (int k = 0; k < T; ++k) {
+                    const int q = lane_pinned + 32 * k;
+                    if (q < H) {
+                        put(o + q, __uint_as_float(static_cast<unsigned>(v[k])), first);
+                        put(o + q + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), first);
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < T; ++k) {
+                    const int q = lane_pinned + 32 * k;
+                    const int64_t t = tw - th + q;
+                    if (q < H && t >= 0 && t < a.n_out)
+                        put(o + q, __uint_as_float(static_cast<unsigned>(v[k])), first);
+                    if (q < H && t + hp >= 0 && t + hp < a.n_out)
+                        put(o + q + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), first);
+                }
             }
         }
     }
