@@ -287,22 +287,23 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     // accumulator registers between copies otherwise).  While channel c is added, the window of
     // c+1 is loaded into wn and the metadata word of c+2 is fetched; the cursor (ring2, par2,
     // ch2, st2) points at channel c+2.
-    u64 w[T + 1], wn[T + 1];
+    u64 w[T + 1];
     const unsigned hdr_off = 16 * g;
     mbar_wait(bar_full, 0);
     unsigned m0 = *reinterpret_cast<const unsigned*>(stages + hdr_off);
     unsigned m1 = *reinterpret_cast<const unsigned*>(stages + hdr_off + 4);
-    load_window<T>(w, stages + lane_off + (m0 >> 21) * 8);
-    const unsigned char* st2 = stages;          // stage of channel c+2
-    const unsigned char* p1 = stages + slot_bytes;  // slot of channel c+1 (without the header offset)
+    const unsigned char* p0 = stages;               // slot of channel c (without the header offset)
+    const unsigned char* st2 = stages;              // stage of channel c+2
+    const unsigned char* p1 = stages + slot_bytes;  // slot of channel c+1
     int ring2 = 0, par2 = 0, ch2 = 2, ring0 = 0;
     const int ntot = nstage * kWinCh;
 #pragma unroll 1
     for (int c = 0; c < ntot; ++c) {
-        load_window<T>(wn, p1 + lane_off + (m1 >> 21) * 8);
+        load_window<T>(w, p0 + lane_off + (m0 >> 21) * 8);
         if (ch2 == 0)
             mbar_wait(bar_full + 8u * ring2, par2);
         const unsigned m2 = *reinterpret_cast<const unsigned*>(st2 + hdr_off + 4 * ch2);
+        p0 = p1;
         p1 = st2 + ch2 * slot_bytes;
         channel(w, m0);
         if ((c & (kWinCh - 1)) == kWinCh - 1) {
@@ -319,9 +320,6 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
             }
             st2 = stages + ring2 * stage_bytes;
         }
-#pragma unroll
-        for (int k = 0; k <= T; ++k)
-            w[k] = wn[k];
         m0 = m1;
         m1 = m2;
     }
