@@ -290,8 +290,8 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
     u64 w[T + 1];
     const unsigned hdr_off = 16 * g;
     mbar_wait(bar_full, 0);
-    unsigned m0 = *reinterpret_cast<const unsigned*>(stages + hdr_off);
-    unsigned m1 = *reinterpret_cast<const unsigned*>(stages + hdr_off + 4);
+    uint4 mq = *reinterpret_cast<const uint4*>(stages + hdr_off);  // words of the cursor's stage
+    unsigned m0 = mq.x, m1 = mq.y;
     const unsigned char* p0 = stages;               // slot of channel c (without the header offset)
     const unsigned char* st2 = stages;              // stage of channel c+2
     const unsigned char* p1 = stages + slot_bytes;  // slot of channel c+1
@@ -300,9 +300,11 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, 1)
 #pragma unroll 1
     for (int c = 0; c < ntot; ++c) {
         load_window<T>(w, p0 + lane_off + (m0 >> 21) * 8);
-        if (ch2 == 0)
+        if (ch2 == 0) {  // the cursor enters a new stage: wait for it, fetch its four words at once
             mbar_wait(bar_full + 8u * ring2, par2);
-        const unsigned m2 = *reinterpret_cast<const unsigned*>(st2 + hdr_off + 4 * ch2);
+            mq = *reinterpret_cast<const uint4*>(st2 + hdr_off);
+        }
+        const unsigned m2 = ch2 == 0 ? mq.x : ch2 == 1 ? mq.y : ch2 == 2 ? mq.z : mq.w;
         p0 = p1;
         p1 = st2 + ch2 * slot_bytes;
         channel(w, m0);
@@ -429,6 +431,8 @@ template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_
     const WindowGeom& g = a.geom;
     if (g.T == 9 && g.G == 8 && g.NT == 1)
         return launch_bands<9, 8, 1, OutT>(a, st, launches);
+    if (g.T == 11 && g.G == 8 && g.NT == 1)
+        return launch_bands<11, 8, 1, OutT>(a, st, launches);
     if (g.T == 7 && g.G == 6 && g.NT == 2)
         return launch_bands<7, 6, 2, OutT>(a, st, launches);
     if (g.T == 5 && g.G == 6 && g.NT == 2)

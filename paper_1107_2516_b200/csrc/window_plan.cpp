@@ -27,7 +27,7 @@ namespace dedisp {
 WindowGeom window_default_geom()
 {
     WindowGeom g;
-    g.T = 9;
+    g.T = 11;
     g.G = 8;
     g.NT = 1;
     // development override: DEDISP_WINDOW_GEOM="T,G,NT" (one of the instantiated geometries)
