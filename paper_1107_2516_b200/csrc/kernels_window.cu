@@ -150,13 +150,14 @@ __device__ __forceinline__ void put(int32_t* p, float v, bool first)
 // smem layout: [nst] full barriers | [nst] empty barriers | transpose scratch [NCW][W] u64 |
 //              nst stages of { 128-byte header, kWinCh channel slots }
 template <int T, int G, int NT, typename OutT>
-__global__ void __launch_bounds__((G * NT + 4) * 32, 1)
+__global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0,
                   const int nst, const int slot_bytes)
 {
     constexpr int W = 32 * T, NCW = G * NT, RB = kWinD * G;
     // registers per consumer thread once the producer warp group has released its share
-    constexpr int kPool = (65536 - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
+    // (blocks of 4 consumer warps run two to an SM and share the register file)
+    constexpr int kPool = ((NCW == 4 ? 32768 : 65536) - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
     constexpr int kConsRegs = kPool > 240 ? 240 : kPool;
     static_assert(NCW % 4 == 0, "setmaxnreg works on groups of four warps");
     extern __shared__ __align__(128) unsigned char smem[];
@@ -384,7 +385,7 @@ static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes)
 {
     const int sb = (lmax * 8 + 127) & ~127;
     const int fixed = 256 + g.G * g.NT * g.W() * 8 + 256;
-    const int budget = 227 * 1024 - fixed;
+    const int budget = (g.G * g.NT == 4 ? 113 : 227) * 1024 - fixed;
     const int stage_bytes = kWinHdrWords * 4 + kWinCh * sb;
     int nst = budget / stage_bytes;
     if (nst > 8)
@@ -433,6 +434,8 @@ template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_
         return launch_bands<9, 8, 1, OutT>(a, st, launches);
     if (g.T == 11 && g.G == 8 && g.NT == 1)
         return launch_bands<11, 8, 1, OutT>(a, st, launches);
+    if (g.T == 11 && g.G == 4 && g.NT == 1)
+        return launch_bands<11, 4, 1, OutT>(a, st, launches);
     if (g.T == 7 && g.G == 6 && g.NT == 2)
         return launch_bands<7, 6, 2, OutT>(a, st, launches);
     if (g.T == 5 && g.G == 6 && g.NT == 2)
