@@ -285,15 +285,36 @@ def main():
             dist.destroy_process_group()
         return
 
+    # ---- dominant kernel alone (roofline): CUDA events recorded by the library on the launching
+    # stream around the band launches of the register-window kernel (or all launches of the other
+    # paths), averaged over the same number of steps
+    plan.set_timing(True)
+    kms = []
+    for _ in range(max(3, min(args.steps, 10))):
+        step()
+        kms.append(plan.last_kernel_ms())
+    plan.set_timing(False)
+    kernel_ms = float(np.mean(kms))
+    resolved = plan.resolved_kernel(dd.U8 if cf.dtype == "u8" else dd.F32)
+    kname = {dd.KERNEL_WINDOW: "dedisp::window_kernel (all band launches of one execute)",
+             dd.KERNEL_DIRECT: "dedisp::direct_kernel", dd.KERNEL_NAIVE: "dedisp::naive_kernel"}.get(resolved, "?")
+    if cf.nsub:
+        kname = "dedisp::direct_kernel (subband stage 1 + stage 2)"
+
     pk = peaks()
     props = torch.cuda.get_device_properties(local)
     nsm = props.multi_processor_count
     alu_peak = nsm * 128 * pk["sm_max_mhz"] * 1e6          # adds/s
-    per_gpu = adds / (ms_step * 1e-3)
+    per_gpu = adds / (kernel_ms * 1e-3)
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get("%s:%d" % (args.workload, resolved))
     roof = {"bound": "alu", "achieved": per_gpu / 1e12, "peak": alu_peak / 1e12, "unit": "TFLOP/s",
-            "frac": per_gpu / alu_peak, "traffic": None,
-            "peak_how": "%d SMs x 128 FP32 lanes x %.0f MHz (1 add = 1 flop)" % (nsm, pk["sm_max_mhz"]),
-            "kernel": "brute-force gather-add (%s)" % args.kernel,
+            "frac": per_gpu / alu_peak, "traffic": traffic,
+            "peak_how": "%d SMs x 128 FP32 lanes x %.0f MHz (1 add = 1 flop; DESIGN.md section 6)" % (nsm, pk["sm_max_mhz"]),
+            "kernel": kname, "kernel_ms": kernel_ms, "algorithmic_adds": adds,
+            "frac_of_step": kernel_ms / ms_step,
             "frac_at_observed_clock": (per_gpu / (nsm * 128 * clocks["sm_mhz"] * 1e6)
                                        if clocks and clocks.get("sm_mhz") else None)}
     in_bytes = float(nb) * cf.nchans * n_in * (1 if cf.dtype == "u8" else 4)
@@ -318,7 +339,8 @@ def main():
                            cf.name, cf.nchans, cf.ndm, n_out,
                            ", %d beams, streaming chunk" % nb if streaming else ""),
                        "nchans": cf.nchans, "ndm": cf.ndm, "n_out": n_out, "nbeams": nb,
-                       "max_delay": M, "kernel": args.kernel, "resolved_kernel": plan.resolved_kernel(),
+                       "max_delay": M, "kernel": args.kernel, "resolved_kernel": plan.resolved_kernel(dd.U8 if cf.dtype == "u8" else dd.F32),
+                       "window": plan.window_info() if not cf.nsub else None,
                        "l2": "inputs larger than L2 (%.2f GB in, %.2f GB out per step)" % (in_bytes / 1e9, out_bytes / 1e9),
                        "parallelism": "1 beam per GPU, no collective" if world > 1 else "single GPU"},
             "real_time_factor": n_out * cf.t_samp_ms * 1e-3 / (ms_step * 1e-3),

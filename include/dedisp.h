@@ -201,6 +201,14 @@ DEDISP_API int64_t dedisp_plan_max_chunk(const dedisp_plan *plan, dedisp_dtype d
 /* Number of kernels the last execute/push on this plan launched (bench.py's gpu_launches). */
 DEDISP_API int dedisp_plan_last_launches(const dedisp_plan *plan);
 
+/* Timing of the dominant kernel(s) for roofline reports.  With timing on, every execute / push
+ * records two CUDA events on the caller's stream: around the band launches of the register-window
+ * kernel (its pairify pre-pass excluded) or around all launches of the other paths.
+ * dedisp_plan_last_kernel_ms waits for the second event and returns the elapsed milliseconds of the
+ * last execute; DEDISP_ESTATE if timing was off.  Off by default (no events, no overhead). */
+DEDISP_API dedisp_status dedisp_plan_set_timing(dedisp_plan *plan, int on);
+DEDISP_API dedisp_status dedisp_plan_last_kernel_ms(dedisp_plan *plan, float *ms);
+
 /* Static string for a status code. */
 DEDISP_API const char *dedisp_strerror(dedisp_status status);
 

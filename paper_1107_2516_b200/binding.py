@@ -40,6 +40,8 @@ _SIGS = {
     "dedisp_stream_destroy": (_int, [_vp]),
     "dedisp_plan_max_chunk": (_i64, [_vp, _int, _i64, _int]),
     "dedisp_plan_last_launches": (_int, [_vp]),
+    "dedisp_plan_set_timing": (_int, [_vp, _int]),
+    "dedisp_plan_last_kernel_ms": (_int, [_vp, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
 }
@@ -151,6 +153,15 @@ class Plan:
 
     def max_chunk(self, dtype, mem_bytes, nbeams=1):
         return int(lib().dedisp_plan_max_chunk(self._h, int(dtype), int(mem_bytes), int(nbeams)))
+
+    def set_timing(self, on=True):
+        _check(lib().dedisp_plan_set_timing(self._h, int(bool(on))), "dedisp_plan_set_timing")
+
+    def last_kernel_ms(self):
+        """Device time of the dominant kernel(s) of the last execute (needs set_timing(True))."""
+        v = ctypes.c_float(0.0)
+        _check(lib().dedisp_plan_last_kernel_ms(self._h, ctypes.addressof(v)), "dedisp_plan_last_kernel_ms")
+        return float(v.value)
 
     @property
     def last_launches(self):

@@ -91,6 +91,10 @@ struct dedisp_plan {
     int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr, *d_win_theta = nullptr, *d_win_hdr = nullptr;
     void* d_win_zeros = nullptr;
     DevBuf pairs;
+    // optional timing of the dominant kernel(s) of an execute (dedisp_plan_set_timing)
+    bool timing = false;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    bool ev_valid = false;
 };
 
 struct dedisp_stream {
@@ -190,6 +194,9 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.stage0 = plan->win.stage0.data();
     a.stage_total = plan->win.stage0[plan->win.nband];
     a.theta_max = plan->win.theta_max;
+    a.ev0 = plan->timing ? plan->ev[0] : nullptr;
+    a.ev1 = plan->timing ? plan->ev[1] : nullptr;
+    plan->ev_valid = plan->timing;
     a.nband = plan->win.nband;
     a.band = plan->win.band.data();
     a.geom = plan->win.geom;
@@ -245,6 +252,22 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     int rc = 0;
     if (use_window(plan, dtype))
         return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream);
+    struct Timer {  // the direct / subband kernels are timed as a whole
+        dedisp_plan* p;
+        cudaStream_t st;
+        Timer(dedisp_plan* p_, void* s) : p(p_), st(static_cast<cudaStream_t>(s))
+        {
+            if (p->timing)
+                cudaEventRecord(p->ev[0], st);
+        }
+        ~Timer()
+        {
+            if (p->timing) {
+                cudaEventRecord(p->ev[1], st);
+                p->ev_valid = true;
+            }
+        }
+    } timer(plan, stream);
     if (plan->nsub == 0) {
         pr.in = in;
         pr.out = out;
@@ -406,6 +429,10 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaFree(p->d_win_hdr);
         cudaFree(p->d_win_zeros);
     }
+    if (p->ev[0])
+        cudaEventDestroy(p->ev[0]);
+    if (p->ev[1])
+        cudaEventDestroy(p->ev[1]);
     p->pairs.release();
     p->scratch.release();
     p->host_in.release();
@@ -420,6 +447,34 @@ int dedisp_plan_ndm(const dedisp_plan* p) { return p ? p->ndm : -1; }
 int dedisp_plan_nsub(const dedisp_plan* p) { return p ? p->nsub : -1; }
 int dedisp_plan_nfine(const dedisp_plan* p) { return p ? p->nfine : -1; }
 int dedisp_plan_last_launches(const dedisp_plan* p) { return p ? p->last_launches : -1; }
+
+dedisp_status dedisp_plan_set_timing(dedisp_plan* p, int on)
+{
+    if (!p)
+        return DEDISP_EINVAL;
+    if (on && !p->ev[0]) {
+        if (cudaEventCreate(&p->ev[0]) != cudaSuccess || cudaEventCreate(&p->ev[1]) != cudaSuccess) {
+            cudaGetLastError();
+            return DEDISP_ECUDA;
+        }
+    }
+    p->timing = on != 0;
+    p->ev_valid = false;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_plan_last_kernel_ms(dedisp_plan* p, float* ms)
+{
+    if (!p || !ms)
+        return DEDISP_EINVAL;
+    if (!p->ev_valid)
+        return DEDISP_ESTATE;
+    if (cudaEventSynchronize(p->ev[1]) != cudaSuccess || cudaEventElapsedTime(ms, p->ev[0], p->ev[1]) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ECUDA;
+    }
+    return DEDISP_OK;
+}
 
 dedisp_status dedisp_plan_get_shifts(const dedisp_plan* p, int32_t* host_out)
 {

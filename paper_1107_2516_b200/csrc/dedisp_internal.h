@@ -103,6 +103,7 @@ struct WindowArgs {
     const int32_t* hdr;     // device copy of WindowPlan::hdr
     const void* zeros;      // device, >= lmax pairs of zeros (segments of the padding channels)
     WindowGeom geom;
+    void *ev0, *ev1;  // cudaEvent_t or nullptr: recorded before the first / after the last band launch
 };
 bool window_fits_smem(const WindowPlan& wp);
 int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out);

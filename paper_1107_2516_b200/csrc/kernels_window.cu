@@ -463,7 +463,12 @@ int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess)
         return static_cast<int>(e);
-    return in_t == Elem::F32 ? launch_geom<float>(a, st, launches) : launch_geom<int32_t>(a, st, launches);
+    if (a.ev0)
+        cudaEventRecord(static_cast<cudaEvent_t>(a.ev0), st);
+    const int rc = in_t == Elem::F32 ? launch_geom<float>(a, st, launches) : launch_geom<int32_t>(a, st, launches);
+    if (a.ev1)
+        cudaEventRecord(static_cast<cudaEvent_t>(a.ev1), st);
+    return rc;
 }
 
 }  // namespace dedisp

@@ -108,6 +108,42 @@ def test_scaled_configs(oracle, k, ndm, n_out):
         check_f32(got, ref, sa)
 
 
+@pytest.mark.parametrize("dtype,beams,n_out", [("f32", 1, 100), ("u8", 3, 700), ("f32", 2, 1331)])
+def test_window_kernel_forced(oracle, dtype, beams, n_out):
+    """The register-window kernel on its own: cfg-2 band (many channel bands), a DM count that is
+    not a multiple of the 64-row block, output lengths below / around one warp tile, several beams."""
+    base = synth.configs()[2]
+    cf = synth.scaled(base, dtype=dtype, n_out=n_out, ndm=150, nchans=384)
+    tab, x = make_case(oracle, cf, beams=beams)
+    plan = dd.Plan(**cf.plan_args())
+    info = plan.window_info()
+    assert info["ok"] == 1 and info["nband"] >= 2
+    plan.set_kernel(dd.KERNEL_WINDOW)
+    assert plan.resolved_kernel(dd.U8 if dtype == "u8" else dd.F32) == dd.KERNEL_WINDOW
+    got = plan.execute(to_dev(x), n_out).cpu().numpy()
+    assert plan.last_launches == 1 + info["nband"]
+    for b in range(beams):
+        if dtype == "u8":
+            assert (got[b] == oracle.brute_u8(x[b], tab, n_out)).all()
+        else:
+            ref, sa = oracle.brute_f32(x[b], tab, n_out)
+            check_f32(got[b], ref, sa)
+    # running it again accumulates nothing from the previous call (band 0 overwrites)
+    again = plan.execute(to_dev(x), n_out).cpu().numpy()
+    assert (again == got).all()
+
+
+def test_kernel_timing_hook(oracle):
+    cf = small_cfg()
+    tab, x = make_case(oracle, cf)
+    plan = dd.Plan(**cf.plan_args())
+    with pytest.raises(dd.DedispError):
+        plan.last_kernel_ms()
+    plan.set_timing(True)
+    plan.execute(to_dev(x[0]), cf.n_out)
+    assert plan.last_kernel_ms() > 0.0
+
+
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
 def test_subband_small(oracle, dtype):
     cf = small_cfg(dtype, nchans=128, ndm=96, n_out=2048 + 33, step=0.25, nsub=8, nfine=12)
