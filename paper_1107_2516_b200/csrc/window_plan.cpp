@@ -85,34 +85,60 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
         }
         return true;
     };
-    wp.band.push_back(0);
-    if (!start_band(0))
-        return false;
-    int kmax = 0;
-    for (int c = 1; c < nchans; ++c) {
-        bool split = false;
-        for (size_t k = 0; k < nrow && !split; ++k) {
-            const int diff = rp[k][c] - r0[k][c];
-            const int b = std::max(base[k], diff - 1);
-            nb[k] = b;
-            // infeasible offset, more than two shifts at once, or too many shifts in this band
-            if (b > diff || b - base[k] > 2 || b - theta[k] > kcap)
-                split = true;
+    // greedy split with at most `cap` row shifts per band; false: the table does not fit the kernel
+    auto split = [&](int cap, std::vector<int32_t>& band, int& kmax_out) -> bool {
+        band.assign(1, 0);
+        if (!start_band(0))
+            return false;
+        int km = 0;
+        for (int c = 1; c < nchans; ++c) {
+            bool cut = false;
+            for (size_t k = 0; k < nrow && !cut; ++k) {
+                const int diff = rp[k][c] - r0[k][c];
+                const int b = std::max(base[k], diff - 1);
+                nb[k] = b;
+                // infeasible offset, more than two shifts at once, or too many shifts in this band
+                if (b > diff || b - base[k] > 2 || b - theta[k] > cap)
+                    cut = true;
+            }
+            if (cut) {
+                if (c - band.back() < 4)
+                    return false;  // trials drift apart faster than the kernel can follow
+                band.push_back(c);
+                if (!start_band(c))
+                    return false;
+            } else {
+                for (size_t k = 0; k < nrow; ++k) {
+                    base[k] = nb[k];
+                    km = std::max(km, base[k] - theta[k]);
+                }
+            }
         }
-        if (split) {
-            if (c - wp.band.back() < 4)
-                return false;  // trials drift apart faster than the kernel can follow
-            wp.band.push_back(c);
-            if (!start_band(c))
-                return false;
-        } else {
-            for (size_t k = 0; k < nrow; ++k) {
-                base[k] = nb[k];
-                kmax = std::max(kmax, base[k] - theta[k]);
+        band.push_back(nchans);
+        kmax_out = km;
+        return true;
+    };
+    int kmax = 0;
+    if (!split(kcap, wp.band, kmax))
+        return false;
+    {
+        // balance: the smallest cap that needs no more bands evens out the band lengths and gives
+        // back the slots a looser cap would waste (H = W - kmax)
+        const size_t nb0 = wp.band.size();
+        int lo = 1, hi = kcap;  // invariant: hi works
+        std::vector<int32_t> tb;
+        while (lo < hi) {
+            const int mid = (lo + hi) / 2;
+            int km = 0;
+            if (split(mid, tb, km) && tb.size() <= nb0) {
+                hi = mid;
+                wp.band = tb;
+                kmax = km;
+            } else {
+                lo = mid + 1;
             }
         }
     }
-    wp.band.push_back(nchans);
     wp.nband = static_cast<int>(wp.band.size()) - 1;
     if (wp.nband > 64)
         return false;
