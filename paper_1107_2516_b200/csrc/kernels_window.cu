@@ -89,6 +89,22 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// producer side: polls with a back-off so that the staging thread does not take issue slots from the
+// two consumer warps that share its scheduler
+__device__ __forceinline__ void mbar_wait_backoff(unsigned bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "WAIT_%=:\n"
+        "nanosleep.u32 64;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -216,7 +232,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
                 }
                 if (lane == 0) {
                     if (lap > 0)
-                        mbar_wait(bar_empty + 8u * ring, (lap - 1) & 1);
+                        mbar_wait_backoff(bar_empty + 8u * ring, (lap - 1) & 1);
                     const unsigned dst = smem_u32(stages) + ring * stage_bytes;
                     const unsigned fb = bar_full + 8u * ring;
                     unsigned bytes = kWinHdrWords * 4;
