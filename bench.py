@@ -146,7 +146,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "naive", "direct", "window"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "naive", "direct", "window", "long"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -175,7 +175,7 @@ def main():
 
     plan = dd.Plan(**cf.plan_args())
     plan.set_kernel({"auto": dd.KERNEL_AUTO, "naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT,
-                     "window": dd.KERNEL_WINDOW}[args.kernel])
+                     "window": dd.KERNEL_WINDOW, "long": dd.KERNEL_LONG}[args.kernel])
     M = plan.max_delay
     n_out = cf.n_out
     streaming = cf.nchunks > 1
@@ -289,32 +289,55 @@ def main():
     # stream around the band launches of the register-window kernel (or all launches of the other
     # paths), averaged over the same number of steps
     plan.set_timing(True)
-    kms = []
+    kms, sms = [], []
     for _ in range(max(3, min(args.steps, 10))):
         step()
         kms.append(plan.last_kernel_ms())
+        if cf.nsub:
+            sms.append(plan.last_stage_ms())
     plan.set_timing(False)
     kernel_ms = float(np.mean(kms))
     resolved = plan.resolved_kernel(dd.U8 if cf.dtype == "u8" else dd.F32)
     kname = {dd.KERNEL_WINDOW: "dedisp::window_kernel (all band launches of one execute)",
-             dd.KERNEL_DIRECT: "dedisp::direct_kernel", dd.KERNEL_NAIVE: "dedisp::naive_kernel"}.get(resolved, "?")
-    if cf.nsub:
-        kname = "dedisp::direct_kernel (subband stage 1 + stage 2)"
+             dd.KERNEL_DIRECT: "dedisp::direct_kernel", dd.KERNEL_NAIVE: "dedisp::naive_kernel",
+             dd.KERNEL_LONG: "dedisp::long_kernel"}.get(resolved, "?")
 
     pk = peaks()
     props = torch.cuda.get_device_properties(local)
     nsm = props.multi_processor_count
     alu_peak = nsm * 128 * pk["sm_max_mhz"] * 1e6          # adds/s
-    per_gpu = adds / (kernel_ms * 1e-3)
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get("%s:%d" % (args.workload, resolved))
+    subband = None
+    if cf.nsub:
+        # the two-stage path executes far fewer adds than the brute-force-equivalent count `value`
+        # is quoted in: stage 1 = sum_k (n_out + maxshift2_k) * nchans, stage 2 = ndm * n_out * nsub.
+        # Stage 1 (the dominant kernel) has no reuse between rows: one shared-memory word per add,
+        # so its ceiling is the 128 B/clk/SM shared-memory pipe = a quarter of the add pipe.
+        m2 = plan.subband_shifts()[3].astype(np.float64)
+        s1_adds = float(nb) * float((n_out + m2).sum()) * cf.nchans
+        s2_adds = float(nb) * cf.ndm * float(n_out) * cf.nsub
+        s1_ms, s2_ms = (float(np.mean([v[k] for v in sms])) for k in (0, 1))
+        s2_bytes = float(nb) * (float((n_out + m2).sum()) * cf.nsub * 4 + float(cf.ndm) * n_out * 4)
+        smem_peak = nsm * 32 * pk["sm_max_mhz"] * 1e6
+        kernel_adds, kernel_ms_dom = s1_adds, s1_ms
+        kname = "%s (subband stage 1)" % kname
+        subband = {"stage1_ms": s1_ms, "stage2_ms": s2_ms, "stage1_adds": s1_adds, "stage2_adds": s2_adds,
+                   "actual_adds_per_s": (s1_adds + s2_adds) / (ms_step * 1e-3),
+                   "stage1_smem_pipe": {"peak_adds_per_s": smem_peak, "frac": s1_adds / (s1_ms * 1e-3) / smem_peak,
+                                        "how": "%d SMs x 32 words/clk x %.0f MHz, one word per add" % (nsm, pk["sm_max_mhz"])},
+                   "stage2_hbm": {"algorithmic_bytes": s2_bytes, "achieved_gbs": s2_bytes / (s2_ms * 1e-3) / 1e9,
+                                  "peak_gbs": pk["hbm_gbs"], "frac": s2_bytes / (s2_ms * 1e-3) / 1e9 / pk["hbm_gbs"]}}
+    else:
+        kernel_adds, kernel_ms_dom = adds, kernel_ms
+    per_gpu = kernel_adds / (kernel_ms_dom * 1e-3)
     roof = {"bound": "alu", "achieved": per_gpu / 1e12, "peak": alu_peak / 1e12, "unit": "TFLOP/s",
             "frac": per_gpu / alu_peak, "traffic": traffic,
             "peak_how": "%d SMs x 128 FP32 lanes x %.0f MHz (1 add = 1 flop; DESIGN.md section 6)" % (nsm, pk["sm_max_mhz"]),
-            "kernel": kname, "kernel_ms": kernel_ms, "algorithmic_adds": adds,
-            "frac_of_step": kernel_ms / ms_step,
+            "kernel": kname, "kernel_ms": kernel_ms_dom, "algorithmic_adds": kernel_adds,
+            "frac_of_step": kernel_ms_dom / ms_step,
             "frac_at_observed_clock": (per_gpu / (nsm * 128 * clocks["sm_mhz"] * 1e6)
                                        if clocks and clocks.get("sm_mhz") else None)}
     in_bytes = float(nb) * cf.nchans * n_in * (1 if cf.dtype == "u8" else 4)
@@ -344,7 +367,7 @@ def main():
                        "l2": "inputs larger than L2 (%.2f GB in, %.2f GB out per step)" % (in_bytes / 1e9, out_bytes / 1e9),
                        "parallelism": "1 beam per GPU, no collective" if world > 1 else "single GPU"},
             "real_time_factor": n_out * cf.t_samp_ms * 1e-3 / (ms_step * 1e-3),
-            "roofline": roof, "hbm": hbm, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roof, "subband": subband, "hbm": hbm, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
             "paper_context": "paper: 50-200x over one Xeon 2.7 GHz core on a Tesla C1060 (PAPER.md:203), ~1.5e10 adds/s",
             "input_gen_s": t_gen}

@@ -57,13 +57,15 @@ typedef enum {
     DEDISP_U8 = 1   /* uint8 input (0..255, no offset removed), int32 output, exact       */
 } dedisp_dtype;
 
-/* Kernel choice for dedisp_plan_set_kernel (brute-force plans).  AUTO picks the register-window
- * kernel when the plan's shift table fits its limits and the direct kernel otherwise. */
+/* Kernel choice for dedisp_plan_set_kernel.  AUTO picks, for brute-force plans, the register-window
+ * kernel when the plan's shift table fits its limits; otherwise, and for both stages of subband
+ * plans, the long-tile kernel (rows of >= 4096 samples) or the direct kernel (shorter rows). */
 typedef enum {
     DEDISP_KERNEL_AUTO = 0,
     DEDISP_KERNEL_NAIVE = 1,  /* one thread per output sample, global loads only (debug)    */
     DEDISP_KERNEL_DIRECT = 2, /* shared-memory staged, register-blocked DMs x time           */
-    DEDISP_KERNEL_WINDOW = 3  /* + one register window shared by the DM rows of a thread     */
+    DEDISP_KERNEL_WINDOW = 3, /* + one register window shared by the DM rows of a thread     */
+    DEDISP_KERNEL_LONG = 4    /* 16 rows x 2048 samples per block, TMA-staged channel unions  */
 } dedisp_kernel;
 
 /*
@@ -208,6 +210,10 @@ DEDISP_API int dedisp_plan_last_launches(const dedisp_plan *plan);
  * last execute; DEDISP_ESTATE if timing was off.  Off by default (no events, no overhead). */
 DEDISP_API dedisp_status dedisp_plan_set_timing(dedisp_plan *plan, int on);
 DEDISP_API dedisp_status dedisp_plan_last_kernel_ms(dedisp_plan *plan, float *ms);
+/* Subband plans, timing on: ms[0] = stage 1 (partial sums inside subbands),
+ * ms[1] = stage 2 (across subbands) of the last execute; HOST, 2 floats.  DEDISP_ESTATE for
+ * brute-force plans or when timing was off. */
+DEDISP_API dedisp_status dedisp_plan_last_stage_ms(dedisp_plan *plan, float *ms);
 
 /* Static string for a status code. */
 DEDISP_API const char *dedisp_strerror(dedisp_status status);

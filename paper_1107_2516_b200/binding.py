@@ -13,7 +13,7 @@ LIB_PATH = os.path.join(_HERE, "libdedisp_b200.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ESHAPE, ESTATE = range(6)
 F32, U8 = 0, 1
-KERNEL_AUTO, KERNEL_NAIVE, KERNEL_DIRECT, KERNEL_WINDOW = range(4)
+KERNEL_AUTO, KERNEL_NAIVE, KERNEL_DIRECT, KERNEL_WINDOW, KERNEL_LONG = range(5)
 
 _c = ctypes
 _vp, _i64, _int, _dbl = _c.c_void_p, _c.c_int64, _c.c_int, _c.c_double
@@ -42,6 +42,7 @@ _SIGS = {
     "dedisp_plan_last_launches": (_int, [_vp]),
     "dedisp_plan_set_timing": (_int, [_vp, _int]),
     "dedisp_plan_last_kernel_ms": (_int, [_vp, _vp]),
+    "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
 }
@@ -162,6 +163,12 @@ class Plan:
         v = ctypes.c_float(0.0)
         _check(lib().dedisp_plan_last_kernel_ms(self._h, ctypes.addressof(v)), "dedisp_plan_last_kernel_ms")
         return float(v.value)
+
+    def last_stage_ms(self):
+        """Subband plans: (stage 1 ms, stage 2 ms) of the last execute (needs set_timing(True))."""
+        v = (ctypes.c_float * 2)()
+        _check(lib().dedisp_plan_last_stage_ms(self._h, ctypes.addressof(v)), "dedisp_plan_last_stage_ms")
+        return float(v[0]), float(v[1])
 
     @property
     def last_launches(self):

@@ -93,8 +93,8 @@ struct dedisp_plan {
     DevBuf pairs;
     // optional timing of the dominant kernel(s) of an execute (dedisp_plan_set_timing)
     bool timing = false;
-    cudaEvent_t ev[2] = {nullptr, nullptr};
-    bool ev_valid = false;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // start, end, between the subband stages
+    bool ev_valid = false, ev_mid_valid = false;
 };
 
 struct dedisp_stream {
@@ -218,7 +218,17 @@ int run_problem(dedisp_plan* plan, const Problem& pr, Elem in_t, const int sprea
 {
     switch (plan->kernel) {
     case DEDISP_KERNEL_NAIVE: return launch_naive(pr, in_t, stream, &plan->last_launches);
-    default: return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
+    case DEDISP_KERNEL_DIRECT: return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
+    default: {
+        // long tiles pay once a row has a few tiles' worth of samples; short problems keep the
+        // 256-sample tiles of the direct kernel
+        if (plan->kernel == DEDISP_KERNEL_LONG || pr.n_out >= 4096) {
+            const int rc = launch_long(pr, in_t, spread[1], stream, &plan->last_launches);
+            if (rc != -1)
+                return rc;
+        }
+        return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
+    }
     }
 }
 
@@ -314,6 +324,11 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     rc = run_problem(plan, pr, in_t, plan->spread_s1, stream);
     if (rc != 0)
         return DEDISP_ECUDA;
+    plan->ev_mid_valid = false;
+    if (plan->timing) {
+        cudaEventRecord(plan->ev[2], static_cast<cudaStream_t>(stream));
+        plan->ev_mid_valid = true;
+    }
     // stage 2: b1 = coarse group k, rows = its nfine trials, channels = the nsub partial series
     Problem p2;
     std::memset(&p2, 0, sizeof(p2));
@@ -433,6 +448,8 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaEventDestroy(p->ev[0]);
     if (p->ev[1])
         cudaEventDestroy(p->ev[1]);
+    if (p->ev[2])
+        cudaEventDestroy(p->ev[2]);
     p->pairs.release();
     p->scratch.release();
     p->host_in.release();
@@ -453,13 +470,29 @@ dedisp_status dedisp_plan_set_timing(dedisp_plan* p, int on)
     if (!p)
         return DEDISP_EINVAL;
     if (on && !p->ev[0]) {
-        if (cudaEventCreate(&p->ev[0]) != cudaSuccess || cudaEventCreate(&p->ev[1]) != cudaSuccess) {
+        if (cudaEventCreate(&p->ev[0]) != cudaSuccess || cudaEventCreate(&p->ev[1]) != cudaSuccess ||
+            cudaEventCreate(&p->ev[2]) != cudaSuccess) {
             cudaGetLastError();
             return DEDISP_ECUDA;
         }
     }
     p->timing = on != 0;
-    p->ev_valid = false;
+    p->ev_valid = p->ev_mid_valid = false;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_plan_last_stage_ms(dedisp_plan* p, float* ms)
+{
+    if (!p || !ms)
+        return DEDISP_EINVAL;
+    if (p->nsub == 0 || !p->ev_valid || !p->ev_mid_valid)
+        return DEDISP_ESTATE;
+    if (cudaEventSynchronize(p->ev[1]) != cudaSuccess ||
+        cudaEventElapsedTime(&ms[0], p->ev[0], p->ev[2]) != cudaSuccess ||
+        cudaEventElapsedTime(&ms[1], p->ev[2], p->ev[1]) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ECUDA;
+    }
     return DEDISP_OK;
 }
 
@@ -504,7 +537,7 @@ dedisp_status dedisp_plan_get_subband_shifts(const dedisp_plan* p, int32_t* s1, 
 
 dedisp_status dedisp_plan_set_kernel(dedisp_plan* p, dedisp_kernel k)
 {
-    if (!p || k < DEDISP_KERNEL_AUTO || k > DEDISP_KERNEL_WINDOW)
+    if (!p || k < DEDISP_KERNEL_AUTO || k > DEDISP_KERNEL_LONG)
         return DEDISP_EINVAL;
     if (k == DEDISP_KERNEL_WINDOW && !(p->nsub == 0 && p->win.ok && p->win_fits))
         return DEDISP_ESTATE;  // the shift table does not fit the register-window kernel's limits
@@ -518,7 +551,8 @@ int dedisp_plan_resolved_kernel(const dedisp_plan* p, dedisp_dtype dtype)
         return -1;
     if (use_window(p, dtype))
         return DEDISP_KERNEL_WINDOW;
-    return p->kernel == DEDISP_KERNEL_AUTO ? DEDISP_KERNEL_DIRECT : p->kernel;
+    // AUTO without the window kernel: long tiles (the direct kernel below 4096 samples per row)
+    return p->kernel == DEDISP_KERNEL_AUTO || p->kernel == DEDISP_KERNEL_WINDOW ? DEDISP_KERNEL_LONG : p->kernel;
 }
 
 dedisp_status dedisp_plan_window_info(const dedisp_plan* p, int64_t* info)

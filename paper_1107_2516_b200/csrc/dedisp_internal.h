@@ -46,6 +46,9 @@ int launch_naive(const Problem& p, Elem in_t, void* stream, int* launches);
 // (max shift - min shift) inside a tile; decides how many rows share one staged copy.
 int launch_direct(const Problem& p, Elem in_t, const int spread[3], void* stream, int* launches);
 
+// kernels_long.cu: 16 rows x 2048 samples per block; spread16 as spread[1] above.  -1: does not fit.
+int launch_long(const Problem& p, Elem in_t, int spread16, void* stream, int* launches);
+
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
 // Geometry: a consumer warp owns the kWinD = 8 DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one

@@ -10,7 +10,8 @@ from paper_1107_2516_b200 import synth, build as ddbuild
 torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
-KERNELS = {"naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT, "auto": dd.KERNEL_AUTO}
+KERNELS = {"naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT, "auto": dd.KERNEL_AUTO,
+           "long": dd.KERNEL_LONG}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -52,7 +53,7 @@ def make_case(oracle, cf, n_out=None, beams=1):
     return tab, np.stack(xs)
 
 
-@pytest.mark.parametrize("kernel", ["naive", "direct", "auto"])
+@pytest.mark.parametrize("kernel", ["naive", "direct", "auto", "long"])
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
 def test_brute_small_ragged(oracle, kernel, dtype):
     cf = small_cfg(dtype)
@@ -144,8 +145,9 @@ def test_kernel_timing_hook(oracle):
     assert plan.last_kernel_ms() > 0.0
 
 
+@pytest.mark.parametrize("kernel", ["direct", "long"])
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
-def test_subband_small(oracle, dtype):
+def test_subband_small(oracle, dtype, kernel):
     cf = small_cfg(dtype, nchans=128, ndm=96, n_out=2048 + 33, step=0.25, nsub=8, nfine=12)
     tab = oracle.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list,
                                 cf.nsub, cf.nfine)
@@ -154,9 +156,13 @@ def test_subband_small(oracle, dtype):
     pulses = [(18, 500, 30, 1.5)]
     x = synth.make_input(cf, n_in, pulses, {18: full[18]})
     plan = dd.Plan(**cf.plan_args())
+    plan.set_kernel(KERNELS[kernel])
     assert plan.max_delay == tab.max_delay
+    plan.set_timing(True)
     got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
     assert plan.last_launches == 2
+    s1_ms, s2_ms = plan.last_stage_ms()
+    assert s1_ms > 0.0 and s2_ms > 0.0 and abs(s1_ms + s2_ms - plan.last_kernel_ms()) < 0.05
     ref, sa = oracle.subband(x, tab, cf.n_out)
     if dtype == "u8":
         assert (got == ref).all()
@@ -175,9 +181,11 @@ def test_cfg4_geometry_subband_scaled(oracle):
     full = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
     x = synth.make_input(cf, cf.n_out + int(full.max()))
     plan = dd.Plan(**cf.plan_args())
-    got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
     ref, sa = oracle.subband(x, tab, cf.n_out)
-    check_f32(got, ref, sa)
+    for kernel in ("auto", "direct"):       # auto = the long-tile kernel (rows of >= 4096 samples)
+        plan.set_kernel(KERNELS[kernel])
+        got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+        check_f32(got, ref, sa)
 
 
 @pytest.mark.parametrize("chunk_rel", ["larger", "smaller"])
