@@ -198,7 +198,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     __syncthreads();
 
     const int nch = c_end - c_begin;
-    const int nstage = (nch + kWinCh - 1) / kWinCh;  // the producer stages one more (all padding)
+    const int nstage = (nch + kWinCh - 1) / kWinCh;
     const int stage_total = a.stage_total;
 
     if (warp >= NCW) {
@@ -214,7 +214,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             const int zlen = ((NT - 1) * a.H + W + 2 + 1) & ~1;  // pairs a padding channel must provide
             int pb = 0, pl = 0;  // lane L: (base, len) of channel 32*q + L
             int ring = 0, lap = 0;
-            for (int s = 0; s <= nstage; ++s) {
+            for (int s = 0; s < nstage; ++s) {
                 if ((s & 7) == 0) {  // 8 stages = 32 channels per metadata fetch
                     const int k = s * kWinCh + lane;
                     pb = 0;
@@ -300,47 +300,50 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         acc[0][0] = add2(acc[0][0], w[0] ^ w[T]);
 #endif
     };
-    // One channel per loop iteration (a single copy of the add block: ptxas permutes the
-    // accumulator registers between copies otherwise).  While channel c is added, the window of
-    // c+1 is loaded into wn and the metadata word of c+2 is fetched; the cursor (ring2, par2,
-    // ch2, st2) points at channel c+2.
+    // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
+    // accumulator registers between copies otherwise).  The bookkeeping that runs once per channel
+    // is kept to the window address and the rotation of the stage's four metadata words: every
+    // uniform-datapath instruction in that chain costs its full latency with two warps per scheduler.
+    // The next stage's barrier wait and metadata load are issued behind the first window load of
+    // the current stage.
     u64 w[T + 1];
     const unsigned hdr_off = 16 * g;
     mbar_wait(bar_full, 0);
-    uint4 mq = *reinterpret_cast<const uint4*>(stages + hdr_off);  // words of the cursor's stage
-    unsigned m0 = mq.x, m1 = mq.y;
-    const unsigned char* p0 = stages;               // slot of channel c (without the header offset)
-    const unsigned char* st2 = stages;              // stage of channel c+2
-    const unsigned char* p1 = stages + slot_bytes;  // slot of channel c+1
-    int ring2 = 0, par2 = 0, ch2 = 2, ring0 = 0;
-    const int ntot = nstage * kWinCh;
+    uint4 mq = *reinterpret_cast<const uint4*>(stages + hdr_off);
+    const unsigned char* sbase = stages;
+    int ring = 0;
+    unsigned par = 0;
 #pragma unroll 1
-    for (int c = 0; c < ntot; ++c) {
-        load_window<T>(w, p0 + lane_off + (m0 >> 21) * 8);
-        if (ch2 == 0) {  // the cursor enters a new stage: wait for it, fetch its four words at once
-            mbar_wait(bar_full + 8u * ring2, par2);
-            mq = *reinterpret_cast<const uint4*>(st2 + hdr_off);
+    for (int s = 0; s < nstage; ++s) {
+        int ring_n = ring + 1;
+        unsigned par_n = par;
+        if (ring_n == nst) {
+            ring_n = 0;
+            par_n ^= 1u;
         }
-        const unsigned m2 = ch2 == 0 ? mq.x : ch2 == 1 ? mq.y : ch2 == 2 ? mq.z : mq.w;
-        p0 = p1;
-        p1 = st2 + ch2 * slot_bytes;
-        channel(w, m0);
-        if ((c & (kWinCh - 1)) == kWinCh - 1) {
-            __syncwarp();
-            mbar_arrive_lane0(bar_empty + 8u * ring0, lane_pinned);
-            if (++ring0 == nst)
-                ring0 = 0;
-        }
-        if (++ch2 == kWinCh) {
-            ch2 = 0;
-            if (++ring2 == nst) {
-                ring2 = 0;
-                par2 ^= 1;
+        const unsigned char* sbase_n = stages + ring_n * stage_bytes;
+        const unsigned char* sp = sbase + lane_off;
+        uint4 mqn = mq;
+        unsigned m = mq.x;
+#pragma unroll 1
+        for (int ch = 0; ch < kWinCh; ++ch) {
+            load_window<T>(w, sp + (m >> 21) * 8);
+            if (ch == 0 && s + 1 < nstage) {
+                mbar_wait(bar_full + 8u * ring_n, par_n);
+                mqn = *reinterpret_cast<const uint4*>(sbase_n + hdr_off);
             }
-            st2 = stages + ring2 * stage_bytes;
+            channel(w, m);
+            sp += slot_bytes;
+            m = mq.y;
+            mq.y = mq.z;
+            mq.z = mq.w;
         }
-        m0 = m1;
-        m1 = m2;
+        __syncwarp();
+        mbar_arrive_lane0(bar_empty + 8u * ring, lane_pinned);
+        ring = ring_n;
+        par = par_n;
+        sbase = sbase_n;
+        mq = mqn;
     }
 
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
