@@ -89,21 +89,17 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
-// producer side: polls with a back-off so that the staging thread does not take issue slots from the
-// two consumer warps that share its scheduler
+// producer side: the staging thread shares its scheduler with two consumer warps, so it must not
+// spin: try_wait with a suspend-time hint parks the thread in hardware between polls
 __device__ __forceinline__ void mbar_wait_backoff(unsigned bar, unsigned parity)
 {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
         "WAIT_%=:\n"
-        "nanosleep.u32 64;\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@!p bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(bar), "r"(parity) : "memory");
+        "}\n" ::"r"(bar), "r"(parity), "r"(20000u) : "memory");
 }
 __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned bytes, unsigned bar)
 {
