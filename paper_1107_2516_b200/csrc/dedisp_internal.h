@@ -50,11 +50,11 @@ int launch_direct(const Problem& p, Elem in_t, const int spread[3], void* stream
 int launch_long(const Problem& p, Elem in_t, int spread16, void* stream, int* launches);
 
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
-// Geometry: a consumer warp owns the kWinD = 8 DM rows of one
+// Geometry: a consumer warp owns the D (4 or 8) DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
 // pair of output samples (t, t + NT*H).  A block has G row groups x NT warps along time
 // (+ 1 producer warp); the channel loop is cut into bands, one launch per band.
-constexpr int kWinD = 8;            // DM rows per thread
+constexpr int kWinD = 8;            // most DM rows per thread (metadata word: 7 bits per mask)
 constexpr int kWinMetaWords = 16;   // per (DM tile, channel) metadata, 64 bytes
 constexpr int kWinWbBits = 11;
 constexpr int kWinCh = 4;           // channels per pipeline stage (one mbarrier pair per stage)
@@ -64,8 +64,9 @@ struct WindowGeom {
     int T = 0;   // slots per lane and row (odd: conflict-free LDS.64)
     int G = 0;   // row groups per block (<= 8)
     int NT = 0;  // warps along time per row group
+    int D = 8;   // DM rows per thread (row group): 8 with T <= 11, 4 with T <= 21
     int W() const { return 32 * T; }
-    int rows() const { return kWinD * G; }
+    int rows() const { return D * G; }
 };
 
 struct WindowPlan {

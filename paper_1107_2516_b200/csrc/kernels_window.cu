@@ -121,10 +121,10 @@ __device__ __forceinline__ u64 add2(u64 a, u64 b)
 // ------------------------------------------------------------------------------------------------
 
 // the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one
-template <int T> __device__ __forceinline__ void shift_rows(u64 (&acc)[kWinD][T], unsigned mask, int lane)
+template <int T, int D> __device__ __forceinline__ void shift_rows(u64 (&acc)[D][T], unsigned mask, int lane)
 {
 #pragma unroll
-    for (int j = 1; j < kWinD; ++j) {
+    for (int j = 1; j < D; ++j) {
         if (mask & (1u << (j - 1))) {
             const u64 carry = __shfl_up_sync(0xffffffffu, acc[j][T - 1], 1);
             shift_row(acc[j], lane ? carry : 0ull);
@@ -161,12 +161,12 @@ __device__ __forceinline__ void put(int32_t* p, float v, bool first)
 
 // smem layout: [nst] full barriers | [nst] empty barriers | transpose scratch [NCW][W] u64 |
 //              nst stages of { 128-byte header, kWinCh channel slots }
-template <int T, int G, int NT, typename OutT>
+template <int T, int G, int NT, int D, typename OutT>
 __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0,
                   const int nst, const int slot_bytes)
 {
-    constexpr int W = 32 * T, NCW = G * NT, RB = kWinD * G;
+    constexpr int W = 32 * T, NCW = G * NT, RB = D * G;
     // registers per consumer thread once the producer warp group has released its share
     // (blocks of 4 consumer warps run two to an SM and share the register file)
     constexpr int kPool = ((NCW == 4 ? 32768 : 65536) - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
@@ -266,12 +266,12 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     int lane_pinned;  // volatile: not rematerialised (S2R) inside the channel loop
     asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane_pinned));
     // lanes 0..7 fetch the flush parameters of rows 0..7 now, long before they are needed
-    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
-    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * kWinD;
-    const int kf_lane = __ldg(kfp + (lane_pinned & 7)), th_lane = __ldg(thp + (lane_pinned & 7));
-    u64 acc[kWinD][T];
+    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
+    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
+    const int kf_lane = __ldg(kfp + (lane_pinned & (D - 1))), th_lane = __ldg(thp + (lane_pinned & (D - 1)));
+    u64 acc[D][T];
 #pragma unroll
-    for (int j = 0; j < kWinD; ++j)
+    for (int j = 0; j < D; ++j)
 #pragma unroll
         for (int i = 0; i < T; ++i)
             acc[j][i] = 0ull;
@@ -283,9 +283,9 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     auto channel = [&](u64(&w)[T + 1], unsigned m) {
         const unsigned sm = (m >> 7) & 0x3fffu;
         if (sm) {
-            shift_rows<T>(acc, sm & 127u, lane_pinned);
+            shift_rows<T, D>(acc, sm & 127u, lane_pinned);
             if (sm >> 7)
-                shift_rows<T>(acc, sm >> 7, lane_pinned);
+                shift_rows<T, D>(acc, sm >> 7, lane_pinned);
         }
 #ifndef DEDISP_EXP_NOMATH
 #pragma unroll
@@ -352,8 +352,8 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // every sample of this warp's two output ranges inside [0, n_out): no bounds tests
     const bool inside = tw - a.theta_max >= 0 && tw + hp + H <= a.n_out;
 #pragma unroll
-    for (int j = 0; j < kWinD; ++j) {
-        const int d = ty * RB + g * kWinD + j;
+    for (int j = 0; j < D; ++j) {
+        const int d = ty * RB + g * D + j;
         const int kf = __shfl_sync(0xffffffffu, kf_lane, j), th = __shfl_sync(0xffffffffu, th_lane, j);
         __syncwarp();
 #pragma unroll
@@ -415,7 +415,7 @@ bool window_fits_smem(const WindowPlan& wp)
     return wp.ok && window_ring(wp.geom, wp.lmax, &sb) > 0;
 }
 
-template <int T, int G, int NT, typename OutT>
+template <int T, int G, int NT, int D, typename OutT>
 static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
 {
     int slot_bytes = 0;
@@ -426,13 +426,13 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     const int stages_off = (tr_off + G * NT * 32 * T * 8 + 127) & ~127;
     const size_t smem = static_cast<size_t>(stages_off) +
                         static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
-    cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, D, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
         return static_cast<int>(e);
     dim3 grid(a.ntile_dm, a.ntile_t, a.nbeams);
     for (int b = 0; b < a.nband; ++b) {
-        window_kernel<T, G, NT, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b,
+        window_kernel<T, G, NT, D, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b,
                                                                               a.stage0[b], nst, slot_bytes);
         ++*launches;
         e = cudaGetLastError();
@@ -445,18 +445,19 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
 template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_t st, int* launches)
 {
     const WindowGeom& g = a.geom;
-    if (g.T == 9 && g.G == 8 && g.NT == 1)
-        return launch_bands<9, 8, 1, OutT>(a, st, launches);
-    if (g.T == 11 && g.G == 8 && g.NT == 1)
-        return launch_bands<11, 8, 1, OutT>(a, st, launches);
-    if (g.T == 11 && g.G == 4 && g.NT == 1)
-        return launch_bands<11, 4, 1, OutT>(a, st, launches);
-    if (g.T == 7 && g.G == 6 && g.NT == 2)
-        return launch_bands<7, 6, 2, OutT>(a, st, launches);
-    if (g.T == 5 && g.G == 6 && g.NT == 2)
-        return launch_bands<5, 6, 2, OutT>(a, st, launches);
-    if (g.T == 7 && g.G == 4 && g.NT == 3)
-        return launch_bands<7, 4, 3, OutT>(a, st, launches);
+#define DEDISP_GEOM(t, gg, nt, dd) \
+    if (g.T == t && g.G == gg && g.NT == nt && g.D == dd) \
+        return launch_bands<t, gg, nt, dd, OutT>(a, st, launches);
+    DEDISP_GEOM(11, 8, 1, 8)
+    DEDISP_GEOM(11, 4, 1, 8)
+    DEDISP_GEOM(9, 8, 1, 8)
+    DEDISP_GEOM(7, 6, 2, 8)
+    DEDISP_GEOM(21, 8, 1, 4)
+    DEDISP_GEOM(19, 8, 1, 4)
+    DEDISP_GEOM(17, 8, 1, 4)
+    DEDISP_GEOM(21, 4, 1, 4)
+    DEDISP_GEOM(19, 4, 1, 4)
+#undef DEDISP_GEOM
     return static_cast<int>(cudaErrorInvalidConfiguration);
 }
 

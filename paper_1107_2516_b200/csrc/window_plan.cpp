@@ -1,6 +1,6 @@
 // Host planner of the register-window kernel (kernels_window.cu).
 //
-// A thread keeps kWinD = 8 DM rows x T output pairs in registers and feeds all rows from ONE
+// A thread keeps D (8 or 4) DM rows x T output pairs in registers and feeds all rows from ONE
 // register window of T + 1 consecutive staged pairs per channel: row j adds w[i + o_j] to its
 // accumulator i, o_j in {0, 1}.  That needs, for every channel c, the samples of the 8 rows to start
 // within one position of a common base.  Neighbouring DM trials drift apart as the frequency drops
@@ -27,16 +27,20 @@ namespace dedisp {
 WindowGeom window_default_geom()
 {
     WindowGeom g;
-    g.T = 11;
-    g.G = 8;
+    // 4 rows x 21 pairs per thread, 4 row groups per block, two blocks per SM: fewer row variants
+    // (branches) per add than 8 x 11 and a slower drift between a thread's rows, so fewer bands
+    g.T = 21;
+    g.G = 4;
     g.NT = 1;
-    // development override: DEDISP_WINDOW_GEOM="T,G,NT" (one of the instantiated geometries)
+    g.D = 4;
+    // development override: DEDISP_WINDOW_GEOM="T,G,NT[,D]" (one of the instantiated geometries)
     if (const char* e = std::getenv("DEDISP_WINDOW_GEOM")) {
-        int t = 0, gg = 0, nt = 0;
-        if (std::sscanf(e, "%d,%d,%d", &t, &gg, &nt) == 3) {
+        int t = 0, gg = 0, nt = 0, dd = 8;
+        if (std::sscanf(e, "%d,%d,%d,%d", &t, &gg, &nt, &dd) >= 3) {
             g.T = t;
             g.G = gg;
             g.NT = nt;
+            g.D = dd;
         }
     }
     return g;
@@ -60,9 +64,10 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
 {
     wp = WindowPlan();
     wp.geom = geom;
-    if (ndm <= 0 || nchans <= 0 || geom.T <= 0 || geom.G <= 0 || geom.G > 8 || geom.NT <= 0)
+    if (ndm <= 0 || nchans <= 0 || geom.T <= 0 || geom.G <= 0 || geom.G > 8 || geom.NT <= 0 || geom.D < 2 ||
+        geom.D > kWinD)
         return false;
-    const int RB = geom.rows(), W = geom.W(), G = geom.G;
+    const int RB = geom.rows(), W = geom.W(), G = geom.G, D = geom.D;
     const int ntile = (ndm + RB - 1) / RB;
     const int kcap = std::max(4, W / 16);
     const Rows R{shift, ndm, nchans, RB};
@@ -74,7 +79,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
     for (int ty = 0; ty < ntile; ++ty)
         for (int r = 0; r < RB; ++r) {
             rp[static_cast<size_t>(ty) * RB + r] = R.row(ty, r);
-            r0[static_cast<size_t>(ty) * RB + r] = R.row(ty, r / kWinD * kWinD);
+            r0[static_cast<size_t>(ty) * RB + r] = R.row(ty, r / D * D);
         }
     auto start_band = [&](int c) -> bool {
         for (size_t k = 0; k < nrow; ++k) {
@@ -163,7 +168,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
                 int32_t* m = wp.meta.data() + (static_cast<size_t>(ty) * nchans + c) * kWinMetaWords;
                 int64_t lo = INT64_MAX, hi = 0;
                 for (int g = 0; g < G; ++g) {
-                    const int64_t om = r0[k0 + g * kWinD][c];
+                    const int64_t om = r0[k0 + g * D][c];
                     lo = std::min(lo, om);
                     hi = std::max(hi, om);
                 }
@@ -177,12 +182,12 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
                 lmax = std::max(lmax, len);
                 maxbase = std::max(maxbase, segbase);
                 for (int g = 0; g < G; ++g) {
-                    const int64_t wb = r0[k0 + g * kWinD][c] - segbase;
+                    const int64_t wb = r0[k0 + g * D][c] - segbase;
                     if (wb + (geom.NT - 1) * H >= (1 << kWinWbBits))
                         return false;
                     unsigned word = static_cast<unsigned>(wb) << 21;
-                    for (int j = 1; j < kWinD; ++j) {
-                        const int r = g * kWinD + j;
+                    for (int j = 1; j < D; ++j) {
+                        const int r = g * D + j;
                         const int diff = rp[k0 + r][c] - r0[k0 + r][c];
                         if (c == wp.band[b])
                             bs[r] = th[r] = std::max(0, diff - 1);
@@ -203,7 +208,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
             }
             for (int r = 0; r < RB; ++r) {
                 const size_t k = (static_cast<size_t>(ty) * wp.nband + b) * RB + r;
-                const bool ref = r % kWinD == 0;
+                const bool ref = r % D == 0;
                 wp.kfinal[k] = ref ? 0 : bs[r] - th[r];
                 wp.theta[k] = ref ? 0 : th[r];
                 theta_max = std::max(theta_max, wp.theta[k]);

@@ -109,16 +109,18 @@ def test_scaled_configs(oracle, k, ndm, n_out):
         check_f32(got, ref, sa)
 
 
-@pytest.mark.parametrize("dtype,beams,n_out", [("f32", 1, 100), ("u8", 3, 700), ("f32", 2, 1331)])
-def test_window_kernel_forced(oracle, dtype, beams, n_out):
-    """The register-window kernel on its own: cfg-2 band (many channel bands), a DM count that is
-    not a multiple of the 64-row block, output lengths below / around one warp tile, several beams."""
+@pytest.mark.parametrize("dtype,beams,n_out,nchans", [("f32", 1, 100, 384), ("u8", 3, 700, 384),
+                                                       ("f32", 2, 1331, 384), ("f32", 1, 1500, 1024)])
+def test_window_kernel_forced(oracle, dtype, beams, n_out, nchans):
+    """The register-window kernel on its own: cfg-2 band, a DM count that is not a multiple of the
+    block's rows, output lengths below / around one warp tile, several beams; the 1024-channel case
+    needs several channel bands (accumulating launches)."""
     base = synth.configs()[2]
-    cf = synth.scaled(base, dtype=dtype, n_out=n_out, ndm=150, nchans=384)
+    cf = synth.scaled(base, dtype=dtype, n_out=n_out, ndm=150, nchans=nchans)
     tab, x = make_case(oracle, cf, beams=beams)
     plan = dd.Plan(**cf.plan_args())
     info = plan.window_info()
-    assert info["ok"] == 1 and info["nband"] >= 2
+    assert info["ok"] == 1 and info["nband"] >= (2 if nchans == 1024 else 1)
     plan.set_kernel(dd.KERNEL_WINDOW)
     assert plan.resolved_kernel(dd.U8 if dtype == "u8" else dd.F32) == dd.KERNEL_WINDOW
     got = plan.execute(to_dev(x), n_out).cpu().numpy()
