@@ -159,8 +159,8 @@ __device__ __forceinline__ void put(int32_t* p, float v, bool first)
         asm volatile("red.global.add.s32 [%0], %1;" ::"l"(p), "r"(iv) : "memory");
 }
 
-// smem layout: [nst] full barriers | [nst] empty barriers | transpose scratch [NCW][W] u64 |
-//              nst stages of { 128-byte header, kWinCh channel slots }
+// smem layout: [nst] full barriers | [nst] empty barriers | nst stages of { 128-byte header, kWinCh
+//              channel slots }; the flush's transpose scratch [NCW][W] u64 overlays the stages
 template <int T, int G, int NT, int D, typename OutT>
 __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0,
@@ -179,8 +179,9 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
 
     const unsigned bar_full = smem_u32(smem);
     const unsigned bar_empty = bar_full + 8u * nst;
-    const int tr_off = (16 * nst + 127) & ~127;
-    const int stages_off = (tr_off + NCW * W * 8 + 127) & ~127;
+    // the flush's transpose scratch [NCW][W] u64 reuses the ring once every consumer has left the loop
+    const int stages_off = (16 * nst + 127) & ~127;
+    const int tr_off = stages_off;
     const int stage_bytes = kWinHdrWords * 4 + kWinCh * slot_bytes;
     unsigned char* stages = smem + stages_off;
 
@@ -343,6 +344,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     }
 
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
+    asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");  // consumers only: the ring is free now
     u64* tr = reinterpret_cast<u64*>(smem + tr_off) + warp * W;
     const bool first = band == 0;
     OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
@@ -399,13 +401,15 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
 static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes)
 {
     const int sb = (lmax * 8 + 127) & ~127;
-    const int fixed = 256 + g.G * g.NT * g.W() * 8 + 256;
+    const int fixed = 256 + 256;  // barriers; the transpose scratch aliases the ring (3 stages > [NCW][W] u64)
     const int budget = (g.G * g.NT == 4 ? 113 : 227) * 1024 - fixed;
     const int stage_bytes = kWinHdrWords * 4 + kWinCh * sb;
     int nst = budget / stage_bytes;
     if (nst > 8)
         nst = 8;
     *slot_bytes = sb;
+    if (nst * stage_bytes < g.G * g.NT * g.W() * 8)
+        return 0;
     return nst >= 3 ? nst : 0;
 }
 
@@ -422,8 +426,7 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     const int nst = window_ring(a.geom, a.lmax, &slot_bytes);
     if (nst == 0)
         return static_cast<int>(cudaErrorInvalidConfiguration);
-    const int tr_off = (16 * nst + 127) & ~127;
-    const int stages_off = (tr_off + G * NT * 32 * T * 8 + 127) & ~127;
+    const int stages_off = (16 * nst + 127) & ~127;
     const size_t smem = static_cast<size_t>(stages_off) +
                         static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
     cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, D, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
