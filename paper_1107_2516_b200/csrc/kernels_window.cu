@@ -269,7 +269,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // lanes 0..7 fetch the flush parameters of rows 0..7 now, long before they are needed
     const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
     const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
-    const int kf_lane = __ldg(kfp + (lane_pinned & (D - 1))), th_lane = __ldg(thp + (lane_pinned & (D - 1)));
+    const int kf_lane = __ldg(kfp + lane_pinned % D), th_lane = __ldg(thp + lane_pinned % D);
     u64 acc[D][T];
 #pragma unroll
     for (int j = 0; j < D; ++j)
@@ -451,15 +451,13 @@ template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_
 #define DEDISP_GEOM(t, gg, nt, dd) \
     if (g.T == t && g.G == gg && g.NT == nt && g.D == dd) \
         return launch_bands<t, gg, nt, dd, OutT>(a, st, launches);
-    DEDISP_GEOM(11, 8, 1, 8)
-    DEDISP_GEOM(11, 4, 1, 8)
-    DEDISP_GEOM(9, 8, 1, 8)
-    DEDISP_GEOM(7, 6, 2, 8)
-    DEDISP_GEOM(21, 8, 1, 4)
-    DEDISP_GEOM(19, 8, 1, 4)
-    DEDISP_GEOM(17, 8, 1, 4)
     DEDISP_GEOM(21, 4, 1, 4)
+    DEDISP_GEOM(21, 8, 1, 4)
     DEDISP_GEOM(19, 4, 1, 4)
+    DEDISP_GEOM(17, 4, 1, 5)
+    DEDISP_GEOM(15, 4, 1, 6)
+    DEDISP_GEOM(11, 4, 1, 8)
+    DEDISP_GEOM(11, 8, 1, 8)
 #undef DEDISP_GEOM
     return static_cast<int>(cudaErrorInvalidConfiguration);
 }
