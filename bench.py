@@ -30,7 +30,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_1107_2516_b200 import synth  # noqa: E402  (input generators only, no arithmetic)
+from paper_1107_2516_b200 import shard, synth  # noqa: E402  (input generators / rank bookkeeping, no arithmetic)
 
 METRIC = "DM*sample*channel adds/s"
 UNIT = "adds/s"
@@ -187,7 +187,7 @@ def main():
     t_gen = time.time()
     if streaming:
         n_in = n_out                      # one chunk per step; the driver carries the overlap
-        host = np.stack([synth.make_input(cf, n_in, beam=rank * cf.nbeams + b) for b in range(cf.nbeams)])
+        host = np.stack([synth.make_input(cf, n_in, beam=shard.beam_of(rank, cf.nbeams, b)) for b in range(cf.nbeams)])
     else:
         n_in = n_out + max(M, full_tab_max if cf.nsub else 0)
         if cf.nchans * n_in > (1 << 31):   # cfg4: 9 GB of input -- generate on the device
@@ -242,10 +242,7 @@ def main():
     w1 = time.time()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop(w0, w1) if rank == 0 else None
-    if world > 1:
-        tmax = torch.tensor([ms], device="cuda")
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
+    ms = shard.max_over_ranks(ms, dist if world > 1 else None, "cuda")
     ms_step = ms / args.steps
     adds = adds_per_step(cf, n_out)
     value = adds * world / (ms_step * 1e-3)
@@ -269,10 +266,7 @@ def main():
             e2e_step()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            tt = torch.tensor([dt], device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dt = float(tt.item())
+        dt = shard.max_over_ranks(dt, dist if world > 1 else None, "cuda")
         e2e = {"value": adds * world * ksteps / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(hin.numel() * hin.element_size()),
                "d2h_bytes_per_step": int(hout.numel() * hout.element_size()), "steps": ksteps,

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -95,6 +96,10 @@ struct dedisp_plan {
     bool timing = false;
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // start, end, between the subband stages
     bool ev_valid = false, ev_mid_valid = false;
+    // dedisp_execute_host pipeline: copy streams and per-chunk events (created on first use)
+    static constexpr int kHostChunks = 8;
+    cudaStream_t copy_st[2] = {nullptr, nullptr};  // H2D, D2H
+    cudaEvent_t ev_copy[2 * kHostChunks + 2] = {};
 };
 
 struct dedisp_stream {
@@ -211,6 +216,26 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.lmax = plan->win.lmax;
     a.ntile_dm = plan->win.ntile_dm;
     a.ntile_t = static_cast<int>(window_ntile_t(plan->win, nsamp_out));
+    {
+        // DM tiles per block-order group: a wave of `inflight` blocks = g DM tiles x inflight/g time
+        // tiles reads about g * cols_per_tile + (inflight / g) * tile_cols columns of the pair buffer;
+        // the g that minimises it
+        int nsm = 148;
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, plan->device);
+        const double inflight = nsm * (plan->win.geom.G * plan->win.geom.NT == 4 ? 2.0 : 1.0);
+        const double tile_cols = 2.0 * plan->win.geom.NT * plan->win.H;
+        double mean_last = 0.0;  // mean over channels of the largest delay
+        const int32_t* last = plan->shift.data() + static_cast<size_t>(plan->ndm - 1) * plan->nchans;
+        for (int c = 0; c < plan->nchans; ++c)
+            mean_last += last[c];
+        mean_last /= plan->nchans;
+        const double cols_per_tile = mean_last / plan->win.ntile_dm + 1.0;
+        int g = static_cast<int>(std::sqrt(inflight * tile_cols / cols_per_tile) + 0.5);
+        g = g < 1 ? 1 : g > plan->win.ntile_dm ? plan->win.ntile_dm : g;
+        if (const char* e = std::getenv("DEDISP_WINDOW_DMGROUP"))  // development override
+            g = std::atoi(e) > 0 ? std::atoi(e) : g;
+        a.dm_group = g > plan->win.ntile_dm ? plan->win.ntile_dm : g;
+    }
     return launch_window(a, in_t, stream, &plan->last_launches) == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
@@ -450,6 +475,12 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaEventDestroy(p->ev[1]);
     if (p->ev[2])
         cudaEventDestroy(p->ev[2]);
+    for (auto& e : p->ev_copy)
+        if (e)
+            cudaEventDestroy(e);
+    for (auto& c : p->copy_st)
+        if (c)
+            cudaStreamDestroy(c);
     p->pairs.release();
     p->scratch.release();
     p->host_in.release();
@@ -606,16 +637,81 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
         cudaGetLastError();
         return DEDISP_ENOMEM;
     }
-    if (cudaMemcpy2DAsync(plan->host_in.p, in_stride * es, host_in, n_in * es, n_in * es, rows_in,
-                          cudaMemcpyHostToDevice, st) != cudaSuccess)
+    // Brute-force plans are cut into up to kHostChunks time chunks so that the H2D copy of chunk
+    // i+1, the kernels of chunk i and the D2H copy of chunk i-1 overlap (outputs of different times
+    // are independent; chunk i reads input columns [t_i, t_i + C_i + max_delay)).
+    int nchunk = 1;
+    if (plan->nsub == 0) {
+        nchunk = static_cast<int>(nsamp_out / 32768);
+        nchunk = nchunk < 1 ? 1 : nchunk > dedisp_plan::kHostChunks ? dedisp_plan::kHostChunks : nchunk;
+    }
+    if (nchunk == 1) {
+        if (cudaMemcpy2DAsync(plan->host_in.p, in_stride * es, host_in, n_in * es, n_in * es, rows_in,
+                              cudaMemcpyHostToDevice, st) != cudaSuccess)
+            return DEDISP_ECUDA;
+        dedisp_status s = execute_device(plan, plan->host_in.p, plan->host_out.p, dtype, nsamp_out,
+                                         in_stride, out_stride, nbeams, cuda_stream);
+        if (s != DEDISP_OK)
+            return s;
+        if (cudaMemcpy2DAsync(host_out, nsamp_out * 4, plan->host_out.p, out_stride * 4, nsamp_out * 4,
+                              rows_out, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            return DEDISP_ECUDA;
+        return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
+    }
+    if (!plan->copy_st[0]) {
+        bool ok = cudaStreamCreateWithFlags(&plan->copy_st[0], cudaStreamNonBlocking) == cudaSuccess &&
+                  cudaStreamCreateWithFlags(&plan->copy_st[1], cudaStreamNonBlocking) == cudaSuccess;
+        for (auto& e : plan->ev_copy)
+            ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            return DEDISP_ECUDA;
+        }
+    }
+    cudaStream_t h2d = plan->copy_st[0], d2h = plan->copy_st[1];
+    cudaEvent_t* ev_in = plan->ev_copy;                              // [nchunk] input columns landed
+    cudaEvent_t* ev_ex = plan->ev_copy + dedisp_plan::kHostChunks;   // [nchunk] kernels of the chunk done
+    cudaEvent_t ev_start = plan->ev_copy[2 * dedisp_plan::kHostChunks];
+    cudaEvent_t ev_done = plan->ev_copy[2 * dedisp_plan::kHostChunks + 1];
+    const int64_t csize = round_up((nsamp_out + nchunk - 1) / nchunk, 64);
+    bool ok = cudaEventRecord(ev_start, st) == cudaSuccess &&
+              cudaStreamWaitEvent(h2d, ev_start, 0) == cudaSuccess &&
+              cudaStreamWaitEvent(d2h, ev_start, 0) == cudaSuccess;
+    const char* hin = static_cast<const char*>(host_in);
+    char* din = static_cast<char*>(plan->host_in.p);
+    char* dout = static_cast<char*>(plan->host_out.p);
+    char* hout = static_cast<char*>(host_out);
+    int launches = 0;
+    int64_t col = 0;  // input columns copied so far
+    for (int i = 0; i < nchunk && ok; ++i) {
+        const int64_t t0 = i * csize;
+        if (t0 >= nsamp_out)
+            break;
+        const int64_t cn = nsamp_out - t0 < csize ? nsamp_out - t0 : csize;
+        const int64_t need = t0 + cn + plan->max_delay;  // input columns chunk i reads
+        if (need > col) {
+            ok = cudaMemcpy2DAsync(din + col * es, in_stride * es, hin + col * es, n_in * es, (need - col) * es,
+                                   rows_in, cudaMemcpyHostToDevice, h2d) == cudaSuccess;
+            col = need;
+        }
+        ok = ok && cudaEventRecord(ev_in[i], h2d) == cudaSuccess && cudaStreamWaitEvent(st, ev_in[i], 0) == cudaSuccess;
+        if (!ok)
+            break;
+        const dedisp_status s = execute_device(plan, din + t0 * es, dout + t0 * 4, dtype, cn, in_stride,
+                                               out_stride, nbeams, cuda_stream);
+        if (s != DEDISP_OK)
+            return s;
+        launches += plan->last_launches;
+        ok = cudaEventRecord(ev_ex[i], st) == cudaSuccess && cudaStreamWaitEvent(d2h, ev_ex[i], 0) == cudaSuccess &&
+             cudaMemcpy2DAsync(hout + t0 * 4, nsamp_out * 4, dout + t0 * 4, out_stride * 4, cn * 4, rows_out,
+                               cudaMemcpyDeviceToHost, d2h) == cudaSuccess;
+    }
+    plan->last_launches = launches;
+    ok = ok && cudaEventRecord(ev_done, d2h) == cudaSuccess && cudaStreamWaitEvent(st, ev_done, 0) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
         return DEDISP_ECUDA;
-    dedisp_status s = execute_device(plan, plan->host_in.p, plan->host_out.p, dtype, nsamp_out,
-                                     in_stride, out_stride, nbeams, cuda_stream);
-    if (s != DEDISP_OK)
-        return s;
-    if (cudaMemcpy2DAsync(host_out, nsamp_out * 4, plan->host_out.p, out_stride * 4, nsamp_out * 4,
-                          rows_out, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-        return DEDISP_ECUDA;
+    }
     return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
 }
 

@@ -174,8 +174,20 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     static_assert(NCW % 4 == 0, "setmaxnreg works on groups of four warps");
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int ty = blockIdx.x, beam = blockIdx.z;
-    const int64_t T0 = static_cast<int64_t>(blockIdx.y) * 2 * NT * a.H;
+    // Block order: groups of a.dm_group DM tiles; inside a group all time tiles, DM tile fastest.
+    // The blocks in flight then read neighbouring delays of a few time tiles: the wave's footprint in
+    // the pair buffer fits L2 (DM-fastest over ALL tiles reads a max_delay-wide range per time tile).
+    const int beam = blockIdx.z;
+    int ty, tt;
+    {
+        const int lin = blockIdx.x, per_group = a.dm_group * a.ntile_t;
+        const int grp = lin / per_group, r = lin - grp * per_group;
+        const int g0 = grp * a.dm_group;
+        const int gsz = a.ntile_dm - g0 < a.dm_group ? a.ntile_dm - g0 : a.dm_group;  // last group may be short
+        tt = r / gsz;
+        ty = g0 + r - tt * gsz;
+    }
+    const int64_t T0 = static_cast<int64_t>(tt) * 2 * NT * a.H;
 
     const unsigned bar_full = smem_u32(smem);
     const unsigned bar_empty = bar_full + 8u * nst;
@@ -433,7 +445,7 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
         return static_cast<int>(e);
-    dim3 grid(a.ntile_dm, a.ntile_t, a.nbeams);
+    dim3 grid(static_cast<unsigned>(a.ntile_dm) * a.ntile_t, 1, a.nbeams);
     for (int b = 0; b < a.nband; ++b) {
         window_kernel<T, G, NT, D, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b,
                                                                               a.stage0[b], nst, slot_bytes);

@@ -257,6 +257,21 @@ def test_execute_host_roundtrip(oracle):
         assert (got[b] == oracle.brute_u8(x[b], tab, cf.n_out)).all()
 
 
+def test_execute_host_pipelined_chunks(oracle):
+    """dedisp_execute_host cuts >= 65536 output samples into time chunks whose copies overlap the
+    kernels; ragged last chunk, two beams, bit-exact; pinned and pageable host buffers."""
+    cf = synth.scaled(small_cfg("u8", nchans=64, ndm=40, step=0.5), n_out=3 * 32768 + 1234)
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    got = plan.execute_host(x, cf.n_out)
+    xp = torch.from_numpy(x).pin_memory()
+    outp = torch.empty((2, cf.ndm, cf.n_out), dtype=torch.int32).pin_memory()
+    plan.execute_host(xp, cf.n_out, out=outp)
+    for b in range(2):
+        ref = oracle.brute_u8(x[b], tab, cf.n_out)
+        assert (got[b] == ref).all() and (outp[b].numpy() == ref).all()
+
+
 def test_cfg3_full_size_sampled(oracle):
     """BASELINE cfg 3 at full size in bench.py's launch configuration; 300 outputs sampled over the
     whole (DM, time) plane are recomputed one by one by the oracle's definition."""
