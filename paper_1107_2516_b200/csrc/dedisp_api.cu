@@ -378,6 +378,19 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
+bool ensure_copy_streams(dedisp_plan* plan)
+{
+    if (plan->copy_st[0])
+        return true;
+    bool ok = cudaStreamCreateWithFlags(&plan->copy_st[0], cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&plan->copy_st[1], cudaStreamNonBlocking) == cudaSuccess;
+    for (auto& e : plan->ev_copy)
+        ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok)
+        cudaGetLastError();
+    return ok;
+}
+
 }  // namespace
 
 extern "C" {
@@ -658,16 +671,8 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
             return DEDISP_ECUDA;
         return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
     }
-    if (!plan->copy_st[0]) {
-        bool ok = cudaStreamCreateWithFlags(&plan->copy_st[0], cudaStreamNonBlocking) == cudaSuccess &&
-                  cudaStreamCreateWithFlags(&plan->copy_st[1], cudaStreamNonBlocking) == cudaSuccess;
-        for (auto& e : plan->ev_copy)
-            ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
-        if (!ok) {
-            cudaGetLastError();
-            return DEDISP_ECUDA;
-        }
-    }
+    if (!ensure_copy_streams(plan))
+        return DEDISP_ECUDA;
     cudaStream_t h2d = plan->copy_st[0], d2h = plan->copy_st[1];
     cudaEvent_t* ev_in = plan->ev_copy;                              // [nchunk] input columns landed
     cudaEvent_t* ev_ex = plan->ev_copy + dedisp_plan::kHostChunks;   // [nchunk] kernels of the chunk done
@@ -807,17 +812,69 @@ dedisp_status dedisp_stream_push_host(dedisp_stream* s, const void* host_chunk_i
     const size_t nout = static_cast<size_t>(s->nbeams) * p->ndm * s->chunk * 4;
     if (s->chunk % 4 != 0)
         return DEDISP_ESHAPE;
-    if (s->host_in.ensure(nin) != cudaSuccess || s->host_out.ensure(nout) != cudaSuccess) {
+    if (s->host_out.ensure(nout) != cudaSuccess) {
         cudaGetLastError();
         return DEDISP_ENOMEM;
     }
-    if (cudaMemcpyAsync(s->host_in.p, host_chunk_in, nin, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    if (!s->zeroed) {
+        dedisp_status r = dedisp_stream_reset(s, cuda_stream);
+        if (r != DEDISP_OK)
+            return r;
+    }
+    // The push is cut into time pieces: the H2D copy of piece j+1 (straight into the work buffer,
+    // behind the carry), the kernels of piece j and the D2H copy of piece j-1 overlap.  Piece j
+    // emits outputs [j*C', (j+1)*C') and reads work columns [j*C', (j+1)*C' + max_delay).
+    if (!ensure_copy_streams(p))
         return DEDISP_ECUDA;
-    dedisp_status r = dedisp_stream_push(s, s->host_in.p, s->host_out.p, cuda_stream);
-    if (r != DEDISP_OK)
-        return r;
-    if (cudaMemcpyAsync(host_out, s->host_out.p, nout, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    const int64_t M = p->max_delay, C = s->chunk;
+    int npiece = static_cast<int>(C / 16384);
+    npiece = npiece < 1 ? 1 : npiece > dedisp_plan::kHostChunks ? dedisp_plan::kHostChunks : npiece;
+    const int64_t psize = round_up((C + npiece - 1) / npiece, 64);
+    const size_t rows_in = static_cast<size_t>(s->nbeams) * p->nchans;
+    const size_t rows_out = static_cast<size_t>(s->nbeams) * p->ndm;
+    unsigned char* cur = static_cast<unsigned char*>(s->work[s->cur].p);
+    unsigned char* nxt = static_cast<unsigned char*>(s->work[s->cur ^ 1].p);
+    const unsigned char* hin = static_cast<const unsigned char*>(host_chunk_in);
+    char* dout = static_cast<char*>(s->host_out.p);
+    char* hout = static_cast<char*>(host_out);
+    cudaStream_t h2d = p->copy_st[0], d2h = p->copy_st[1];
+    cudaEvent_t* ev_in = p->ev_copy;
+    cudaEvent_t* ev_ex = p->ev_copy + dedisp_plan::kHostChunks;
+    cudaEvent_t ev_start = p->ev_copy[2 * dedisp_plan::kHostChunks];
+    cudaEvent_t ev_done = p->ev_copy[2 * dedisp_plan::kHostChunks + 1];
+    bool ok = cudaEventRecord(ev_start, st) == cudaSuccess && cudaStreamWaitEvent(h2d, ev_start, 0) == cudaSuccess &&
+              cudaStreamWaitEvent(d2h, ev_start, 0) == cudaSuccess;
+    int launches = 0;
+    for (int j = 0; j < npiece && ok; ++j) {
+        const int64_t t0 = j * psize;
+        if (t0 >= C)
+            break;
+        const int64_t cn = C - t0 < psize ? C - t0 : psize;
+        ok = cudaMemcpy2DAsync(cur + (M + t0) * es, s->wstride * es, hin + t0 * es, C * es, cn * es, rows_in,
+                               cudaMemcpyHostToDevice, h2d) == cudaSuccess &&
+             cudaEventRecord(ev_in[j], h2d) == cudaSuccess && cudaStreamWaitEvent(st, ev_in[j], 0) == cudaSuccess;
+        if (!ok)
+            break;
+        const dedisp_status r = execute_device(p, cur + t0 * es, dout + t0 * 4, s->dtype, cn, s->wstride, C,
+                                               s->nbeams, cuda_stream);
+        if (r != DEDISP_OK)
+            return r;
+        launches += p->last_launches;
+        ok = cudaEventRecord(ev_ex[j], st) == cudaSuccess && cudaStreamWaitEvent(d2h, ev_ex[j], 0) == cudaSuccess &&
+             cudaMemcpy2DAsync(hout + t0 * 4, C * 4, dout + t0 * 4, C * 4, cn * 4, rows_out, cudaMemcpyDeviceToHost,
+                               d2h) == cudaSuccess;
+    }
+    p->last_launches = launches;
+    // the last max_delay samples become the head of the other buffer
+    if (ok && M > 0)
+        ok = cudaMemcpy2DAsync(nxt, s->wstride * es, cur + C * es, s->wstride * es, M * es, rows_in,
+                               cudaMemcpyDeviceToDevice, st) == cudaSuccess;
+    s->cur ^= 1;
+    ok = ok && cudaEventRecord(ev_done, d2h) == cudaSuccess && cudaStreamWaitEvent(st, ev_done, 0) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
         return DEDISP_ECUDA;
+    }
     return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
 }
 

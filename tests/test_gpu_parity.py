@@ -223,6 +223,27 @@ def test_streaming_equals_one_shot(oracle, dtype, chunk_rel):
     plan.close()
 
 
+def test_stream_push_host_pieces(oracle):
+    """dedisp_stream_push_host: host chunks copied straight behind the carry in time pieces that
+    overlap the kernels; three pushes of 2.2 pieces each equal the one-shot result bit for bit."""
+    cf = small_cfg("u8", nchans=48, ndm=24, n_out=0, step=0.6)
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    M, C, npush = int(tab.max()), 2 * 16384 + 3000, 3
+    xs = synth.make_input(cf, npush * C, [(5, M + 50, 9, 2.0)], {5: tab[5]})[None]
+    plan = dd.Plan(**cf.plan_args())
+    st = dd.Stream(plan, dd.U8, C, 1)
+    outs = []
+    for k in range(npush):
+        hin = torch.from_numpy(np.ascontiguousarray(xs[:, :, k * C:(k + 1) * C])).pin_memory()
+        hout = torch.empty((1, cf.ndm, C), dtype=torch.int32).pin_memory()
+        st.push_host(hin, hout)
+        outs.append(hout.numpy().copy())
+    got = np.concatenate(outs, axis=2)[0][:, M:]
+    assert (got == oracle.brute_u8(xs[0], tab, npush * C - M)).all()
+    st.close()
+    plan.close()
+
+
 def test_edge_cases(oracle):
     # one channel, one DM, one sample; DM 0 only; nsamp_out = 0
     p = dd.Plan(1, 100.0, 1.0, 1.0, [0.0])
