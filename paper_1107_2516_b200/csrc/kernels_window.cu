@@ -19,6 +19,7 @@
 //     accumulators go through a per-warp shared-memory transpose to coalesced global accesses:
 //     band 0 stores, later bands add to what is there.
 #include <cuda_runtime.h>
+#include <cstdlib>
 
 #include "dedisp_internal.h"
 
@@ -313,8 +314,8 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // accumulator registers between copies otherwise).  The bookkeeping that runs once per channel
     // is kept to the window address and the rotation of the stage's four metadata words: every
     // uniform-datapath instruction in that chain costs its full latency with two warps per scheduler.
-    // The next stage's barrier wait and metadata load are issued behind the first window load of
-    // the current stage.
+    // The next stage's barrier wait and metadata load sit between two stages, outside the channel
+    // loop: three more bookkeeping instructions per channel cost more than the exposed latency.
     u64 w[T + 1];
     const unsigned hdr_off = 16 * g;
     mbar_wait(bar_full, 0);
@@ -332,15 +333,10 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         }
         const unsigned char* sbase_n = stages + ring_n * stage_bytes;
         const unsigned char* sp = sbase + lane_off;
-        uint4 mqn = mq;
         unsigned m = mq.x;
 #pragma unroll 1
         for (int ch = 0; ch < kWinCh; ++ch) {
             load_window<T>(w, sp + (m >> 21) * 8);
-            if (ch == 0 && s + 1 < nstage) {
-                mbar_wait(bar_full + 8u * ring_n, par_n);
-                mqn = *reinterpret_cast<const uint4*>(sbase_n + hdr_off);
-            }
             channel(w, m);
             sp += slot_bytes;
             m = mq.y;
@@ -349,10 +345,13 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         }
         __syncwarp();
         mbar_arrive_lane0(bar_empty + 8u * ring, lane_pinned);
+        if (s + 1 < nstage) {
+            mbar_wait(bar_full + 8u * ring_n, par_n);
+            mq = *reinterpret_cast<const uint4*>(sbase_n + hdr_off);
+        }
         ring = ring_n;
         par = par_n;
         sbase = sbase_n;
-        mq = mqn;
     }
 
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
@@ -439,8 +438,10 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     if (nst == 0)
         return static_cast<int>(cudaErrorInvalidConfiguration);
     const int stages_off = (16 * nst + 127) & ~127;
-    const size_t smem = static_cast<size_t>(stages_off) +
-                        static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
+    size_t smem = static_cast<size_t>(stages_off) +
+                  static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
+    if (const char* e = getenv("DEDISP_EXP_SMEM_PAD"))
+        smem += atoi(e);
     cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, D, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
