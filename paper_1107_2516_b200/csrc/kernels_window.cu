@@ -295,8 +295,8 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // added (wa / wb alternate).
     const unsigned lane_off = kWinHdrWords * 4 + (wt * a.H + lane_pinned * T) * 8;  // bytes from the slot start
     auto channel = [&](u64(&w)[T + 1], unsigned m) {
-        const unsigned sm = (m >> 7) & 0x3fffu;
-        if (sm) {
+        if (m & 0x1fff80u) {  // any row shift (rare): one test on the word itself
+            const unsigned sm = (m >> 7) & 0x3fffu;
             shift_rows<T, D>(acc, sm & 127u, lane_pinned);
             if (sm >> 7)
                 shift_rows<T, D>(acc, sm >> 7, lane_pinned);
