@@ -294,21 +294,17 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // add the four channels of this stage; the window of channel k+1 is loaded while channel k is
     // added (wa / wb alternate).
     const unsigned lane_off = kWinHdrWords * 4 + (wt * a.H + lane_pinned * T) * 8;  // bytes from the slot start
-    auto channel = [&](u64(&w)[T + 1], unsigned m) {
-        if (m & 0x1fff80u) {  // any row shift (rare): one test on the word itself
-            const unsigned sm = (m >> 7) & 0x3fffu;
-            shift_rows<T, D>(acc, sm & 127u, lane_pinned);
-            if (sm >> 7)
-                shift_rows<T, D>(acc, sm >> 7, lane_pinned);
-        }
-#ifndef DEDISP_EXP_NOMATH
+    auto shifts = [&](unsigned m) {
+        const unsigned sm = (m >> 7) & 0x3fffu;
+        shift_rows<T, D>(acc, sm & 127u, lane_pinned);
+        if (sm >> 7)
+            shift_rows<T, D>(acc, sm >> 7, lane_pinned);
+    };
+    auto adds = [&](u64(&w)[T + 1], unsigned m) {
 #pragma unroll
         for (int k = 0; k < T; ++k)
             acc[0][k] = add2(acc[0][k], w[k]);
         rows7(acc, w, m);
-#else
-        acc[0][0] = add2(acc[0][0], w[0] ^ w[T]);
-#endif
     };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
     // accumulator registers between copies otherwise).  The bookkeeping that runs once per channel
@@ -334,14 +330,29 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         const unsigned char* sbase_n = stages + ring_n * stage_bytes;
         const unsigned char* sp = sbase + lane_off;
         unsigned m = mq.x;
+        if (((mq.x | mq.y) | (mq.z | mq.w)) & 0x1fff80u) {
+            // a row shift somewhere in this stage (about a third of the stages)
 #pragma unroll 1
-        for (int ch = 0; ch < kWinCh; ++ch) {
-            load_window<T>(w, sp + (m >> 21) * 8);
-            channel(w, m);
-            sp += slot_bytes;
-            m = mq.y;
-            mq.y = mq.z;
-            mq.z = mq.w;
+            for (int ch = 0; ch < kWinCh; ++ch) {
+                load_window<T>(w, sp + (m >> 21) * 8);
+                if (m & 0x1fff80u)
+                    shifts(m);
+                adds(w, m);
+                sp += slot_bytes;
+                m = mq.y;
+                mq.y = mq.z;
+                mq.z = mq.w;
+            }
+        } else {
+#pragma unroll 1
+            for (int ch = 0; ch < kWinCh; ++ch) {
+                load_window<T>(w, sp + (m >> 21) * 8);
+                adds(w, m);
+                sp += slot_bytes;
+                m = mq.y;
+                mq.y = mq.z;
+                mq.z = mq.w;
+            }
         }
         __syncwarp();
         mbar_arrive_lane0(bar_empty + 8u * ring, lane_pinned);
