@@ -136,6 +136,39 @@ def test_window_kernel_forced(oracle, dtype, beams, n_out, nchans):
     assert (again == got).all()
 
 
+@pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
+def test_random_plans_all_kernels(oracle, seed):
+    """Seeded random bands, sampling times and DM lists (irregular steps, repeated trials, a DM count
+    that is no multiple of any tile) on uint8 input: every kernel the plan accepts must be bit-exact."""
+    rng = np.random.default_rng(1107_2516 + seed)
+    nchans = int(rng.integers(3, 200))
+    f_top = float(rng.uniform(120.0, 1600.0))
+    df = float(rng.uniform(0.2, 0.9)) * f_top / nchans * 0.3
+    t_samp = float(rng.choice([0.05, 0.064, 0.1, 0.5]))
+    ndm = int(rng.integers(1, 90))
+    kmax = 4.15e6 * ((f_top - (nchans - 1) * df) ** -2 - f_top ** -2) / t_samp   # samples per unit DM
+    steps = rng.uniform(0.0, 2.0, ndm) * (rng.uniform(0.3, 6.0) / max(kmax, 1e-9))
+    steps[rng.random(ndm) < 0.1] = 0.0                                           # repeated trials
+    dm = np.cumsum(steps)
+    n_out = int(rng.integers(1, 3000))
+    tab = oracle.shift_table(nchans, f_top, df, t_samp, dm)
+    x = rng.integers(0, 256, (nchans, n_out + int(tab.max())), dtype=np.uint8)
+    ref = oracle.brute_u8(x, tab, n_out)
+    plan = dd.Plan(nchans, f_top, df, t_samp, dm)
+    assert (plan.shifts() == tab).all()
+    tried = 0
+    for name in ("auto", "direct", "long", "naive", "window"):
+        try:
+            plan.set_kernel(KERNELS.get(name, dd.KERNEL_WINDOW))
+        except dd.DedispError:
+            assert name == "window" and plan.window_info()["ok"] == 0
+            continue
+        got = plan.execute(to_dev(x), n_out).cpu().numpy()
+        assert (got == ref).all(), name
+        tried += 1
+    assert tried >= 4
+
+
 def test_kernel_timing_hook(oracle):
     cf = small_cfg()
     tab, x = make_case(oracle, cf)
