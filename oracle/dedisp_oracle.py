@@ -191,3 +191,21 @@ def subband(x, tab, n_out, groups=None, want_sumabs=True):
         if rc != 0:
             raise ValueError("oracle_subband_stage2: intermediate too short")
     return (out, sa) if want_sumabs else out
+
+
+def detect(out, nsigma):
+    """Event detection on one de-dispersed buffer out[ndm][n]: mean and standard
+    deviation of the ENTIRE buffer, threshold mu + nsigma * sigma, every value above it as a triplet
+    (time, DM trial, intensity).  Readings (R14): population standard deviation (divide by
+    N), strict '>', fp64 statistics.  Returns (mu, sigma, threshold, events) with events an int64
+    array [k][2] of (t, d) sorted by (d, t) and the intensities out[d][t].
+    Pins (tests/test_oracle_pins.py): constant buffer -> no events; one spike of height A in N zeros
+    -> mu = A/N, sigma = A*sqrt(N-1)/N, detected iff sqrt(N-1) > nsigma; Gaussian buffer -> count
+    near N*Q(nsigma); the paper's Fig. 5 statement: the 5-sigma events of a simulated pulsar sit at
+    its DM trial."""
+    x = np.asarray(out, dtype=np.float64)
+    mu = float(x.mean())
+    sigma = float(np.sqrt(((x - mu) ** 2).mean()))
+    thr = mu + float(nsigma) * sigma
+    d, t = np.nonzero(x > thr)
+    return mu, sigma, thr, np.stack([t, d], axis=1).astype(np.int64), np.asarray(out)[d, t]

@@ -366,3 +366,43 @@ def test_p9_chunked_equals_one_shot_on_the_oracle(oracle):
         got = np.concatenate(outs, axis=1)[:, M:]
         n = min(got.shape[1], one.shape[1])
         assert n > 0 and (got[:, :n] == one[:, :n]).all()
+
+
+# ---------------------------------------------------------------- event detection
+def test_detect_closed_forms(oracle):
+    # constant buffer: sigma = 0, nothing is above the mean
+    mu, sg, thr, ev, val = oracle.detect(np.full((7, 33), 4.5, dtype=np.float32), 3.0)
+    assert mu == 4.5 and sg == 0.0 and len(ev) == 0
+    # one spike of height A in N zeros: mu = A/N, sigma = A*sqrt(N-1)/N
+    N, A = 20 * 50, 12.0
+    x = np.zeros((20, 50), dtype=np.float32)
+    x[13, 7] = A
+    mu, sg, thr, ev, val = oracle.detect(x, 5.0)
+    assert np.isclose(mu, A / N) and np.isclose(sg, A * np.sqrt(N - 1) / N)
+    assert ev.tolist() == [[7, 13]] and val.tolist() == [A]          # (time, DM trial)
+    assert len(oracle.detect(x, np.sqrt(N - 1) + 1.0)[3]) == 0        # detected iff sqrt(N-1) > nsigma
+    # two equal spikes, threshold strictly above
+    x[2, 2] = A
+    assert oracle.detect(x, 5.0)[3].tolist() == [[2, 2], [7, 13]]     # sorted by (d, t)
+    # Gaussian buffer: about N * Q(3) = N * 1.35e-3 values above 3 sigma
+    g = np.random.default_rng(5).standard_normal((64, 8192)).astype(np.float32)
+    n3 = len(oracle.detect(g, 3.0)[3])
+    assert abs(n3 - g.size * 1.3499e-3) < 5 * np.sqrt(g.size * 1.3499e-3)
+
+
+def test_detect_paper_fig5_statement(oracle):
+    """PAPER.md:197 (Fig. 5): with a 5-sigma threshold on the de-dispersed output of a simulated
+    pulsar the data points are at the pulsar's DM; Table-2-like input as in the P7 pin."""
+    nch, ft, df, ts = 1024, 156.0, 0.005941, 0.165
+    dm = np.arange(70, 81, dtype=np.float64)            # trial 5 = DM 75
+    cf = synth.Config("fake", nch, ft, df, ts, 2048, dm.size, 1.0, seed=77)
+    tab = oracle.shift_table(nch, ft, df, ts, dm)
+    w = 60
+    pulses = [(5, 500, w, 0.25), (5, 1500, w, 0.25)]
+    x = synth.make_input(cf, cf.n_out + int(tab.max()), pulses, {5: tab[5]}, threads=1)
+    out, _ = oracle.brute_f32(x, tab, cf.n_out)
+    mu, sg, thr, ev, val = oracle.detect(out, 5.0)
+    assert len(ev) > 0.5 * 2 * w                        # most on-pulse samples (S/N 8) pass 5 sigma
+    on = ((ev[:, 0] >= 500) & (ev[:, 0] < 500 + w)) | ((ev[:, 0] >= 1500) & (ev[:, 0] < 1500 + w))
+    assert (ev[on, 1] == 5).mean() > 0.9 and on.mean() > 0.95   # at the true trial, inside the pulses
+    assert (val > thr).all()
