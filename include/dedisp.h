@@ -215,6 +215,30 @@ DEDISP_API dedisp_status dedisp_plan_last_kernel_ms(dedisp_plan *plan, float *ms
  * brute-force plans or when timing was off. */
 DEDISP_API dedisp_status dedisp_plan_last_stage_ms(dedisp_plan *plan, float *ms);
 
+/*
+ * Event detection on a de-dispersed buffer ("calculate the mean and standard deviation
+ * for the entire processed buffer, and use these values to apply a threshold at a particular
+ * multiple of the standard deviation.  All values above the threshold are output ... as a list of
+ * triplets of the form (time, DM, intensity)").  Per beam: mean and POPULATION standard deviation of
+ * all ndm*nsamp_out outputs in fp64, threshold = mean + nsigma*sigma, events = outputs strictly
+ * above it.
+ *
+ *   out        DEVICE, [nbeams][ndm][out_stride] float (DEDISP_F32) or int32 (DEDISP_U8), as written
+ *              by dedisp_execute; 16-byte aligned, out_stride a multiple of 4
+ *   events     DEVICE, [nbeams][capacity]; the first min(count, capacity) entries of a beam are
+ *              valid, in no particular order
+ *   results    DEVICE, [nbeams]; count is the number of outputs above the threshold (it may exceed
+ *              capacity: the surplus is counted, not stored)
+ * Asynchronous on cuda_stream; the plan owns a small workspace (one detect per plan in flight).
+ * Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ENOMEM, DEDISP_ECUDA.
+ */
+typedef struct { int64_t t; int32_t dm; float value; } dedisp_event;            /* 16 bytes */
+typedef struct { double mean, sigma, threshold; int64_t count; } dedisp_detect_result;
+DEDISP_API dedisp_status dedisp_plan_detect(dedisp_plan *plan, const void *out, dedisp_dtype dtype,
+                                            int64_t nsamp_out, int64_t out_stride, int nbeams, double nsigma,
+                                            dedisp_event *events, int64_t capacity,
+                                            dedisp_detect_result *results, void *cuda_stream);
+
 /* Static string for a status code. */
 DEDISP_API const char *dedisp_strerror(dedisp_status status);
 

@@ -43,6 +43,7 @@ _SIGS = {
     "dedisp_plan_set_timing": (_int, [_vp, _int]),
     "dedisp_plan_last_kernel_ms": (_int, [_vp, _vp]),
     "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
+    "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
 }
@@ -198,6 +199,28 @@ class Plan:
                                     int(x3.stride(1)), int(out3.stride(1)), int(nb), _stream_ptr(stream)),
                "dedisp_execute")
         return out3 if x.dim() == 3 else out3[0]
+
+    def detect(self, out, nsigma, capacity=1 << 20, stream=None):
+        """dedisp_plan_detect on a CUDA tensor out[(nbeams,) ndm, n] as returned by execute.  Returns
+        (results, events): per-beam dicts {mean, sigma, threshold, count} and numpy record arrays
+        (t, dm, value) of the stored events (unordered)."""
+        import torch
+        o = out if out.dim() == 3 else out[None]
+        assert o.is_cuda and o.stride(2) == 1 and o.shape[1] == self.ndm and o.stride(0) == o.stride(1) * self.ndm
+        dt = F32 if o.dtype == torch.float32 else U8
+        nb = o.shape[0]
+        ev = torch.zeros((nb, capacity, 4), dtype=torch.int32, device=o.device)     # 16-byte records
+        res = torch.zeros((nb, 4), dtype=torch.float64, device=o.device)            # 32-byte records
+        _check(lib().dedisp_plan_detect(self._h, o.data_ptr(), dt, int(o.shape[2]), int(o.stride(1)), int(nb),
+                                        float(nsigma), ev.data_ptr(), int(capacity), res.data_ptr(),
+                                        _stream_ptr(stream)), "dedisp_plan_detect")
+        rh = res.cpu().numpy()
+        counts = rh[:, 3].copy().view(np.int64)
+        results = [dict(mean=float(rh[b, 0]), sigma=float(rh[b, 1]), threshold=float(rh[b, 2]), count=int(counts[b]))
+                   for b in range(nb)]
+        rec = np.dtype([("t", np.int64), ("dm", np.int32), ("value", np.float32)])
+        events = [ev[b, :min(int(counts[b]), capacity)].cpu().numpy().view(rec).reshape(-1) for b in range(nb)]
+        return results, events
 
     def execute_host(self, x, nsamp_out, out=None, stream=None):
         """x: numpy / CPU tensor [nbeams][nchans][nsamp_out+max_delay] dense; returns numpy out."""

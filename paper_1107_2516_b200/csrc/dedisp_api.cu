@@ -83,6 +83,7 @@ struct dedisp_plan {
     int32_t *d_shift = nullptr, *d_s1 = nullptr, *d_s2 = nullptr, *d_maxshift2 = nullptr;
     DevBuf scratch;            // subband intermediate
     DevBuf host_in, host_out;  // staging for dedisp_execute_host
+    DevBuf det_partial;        // dedisp_plan_detect workspace
     dedisp_kernel kernel = DEDISP_KERNEL_AUTO;
     int last_launches = 0;
     int nstreams = 0;
@@ -498,6 +499,7 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
     p->scratch.release();
     p->host_in.release();
     p->host_out.release();
+    p->det_partial.release();
     delete p;
     return DEDISP_OK;
 }
@@ -906,6 +908,27 @@ int64_t dedisp_plan_max_chunk(const dedisp_plan* p, dedisp_dtype dtype, int64_t 
     if (!(n >= 1.0))
         return 0;
     return static_cast<int64_t>(n) / 16 * 16;
+}
+
+dedisp_status dedisp_plan_detect(dedisp_plan* plan, const void* out, dedisp_dtype dtype, int64_t nsamp_out,
+                                 int64_t out_stride, int nbeams, double nsigma, dedisp_event* events,
+                                 int64_t capacity, dedisp_detect_result* results, void* cuda_stream)
+{
+    if (!plan || !out || !results || nbeams <= 0 || nsamp_out <= 0 || capacity < 0 || (capacity > 0 && !events) ||
+        !(nsigma == nsigma) || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    if (out_stride < nsamp_out || out_stride % 4 != 0 || (reinterpret_cast<uintptr_t>(out) & 15) != 0)
+        return DEDISP_ESHAPE;
+    const size_t need = static_cast<size_t>(nbeams) * detect_blocks(plan->ndm) * 2 * sizeof(double);
+    if (plan->det_partial.ensure(need) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    plan->last_launches = 0;
+    const int rc = launch_detect(out, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, nbeams, plan->ndm, nsamp_out,
+                                 out_stride, nsigma, events, capacity, results,
+                                 static_cast<double*>(plan->det_partial.p), cuda_stream, &plan->last_launches);
+    return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
 const char* dedisp_strerror(dedisp_status s)

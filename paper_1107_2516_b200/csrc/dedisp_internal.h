@@ -49,6 +49,13 @@ int launch_direct(const Problem& p, Elem in_t, const int spread[3], void* stream
 // kernels_long.cu: 16 rows x 2048 samples per block; spread16 as spread[1] above.  -1: does not fit.
 int launch_long(const Problem& p, Elem in_t, int spread16, void* stream, int* launches);
 
+// kernels_detect.cu: statistics, threshold, triplets.  partial: device workspace of
+// nbeams * detect_blocks(ndm) * 2 doubles.
+int detect_blocks(int ndm);
+int launch_detect(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64_t stride, double nsigma,
+                  dedisp_event* events, int64_t capacity, dedisp_detect_result* res, double* partial, void* stream,
+                  int* launches);
+
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
 // Geometry: a consumer warp owns the D (4 or 8) DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one

@@ -1,0 +1,164 @@
+// Event detection on a de-dispersed buffer: mean and standard
+// deviation of the ENTIRE buffer, threshold mu + nsigma * sigma, every value above it emitted as a
+// (time, DM trial, intensity) triplet.  HBM-bound: two passes over out[ndm][n] (statistics, then the
+// threshold scan), 16-byte loads, fp64 sums reduced in a fixed order (per-thread, warp shuffles,
+// per-block partials, one finishing block), so mu, sigma and therefore the event set do not depend
+// on scheduling; only the ORDER of the triplets does (an atomic cursor).
+#include <cuda_runtime.h>
+
+#include "dedisp_internal.h"
+
+namespace dedisp {
+
+namespace {
+
+constexpr int kDetThreads = 256;
+
+template <typename T> __device__ __forceinline__ double to_f64(T v) { return static_cast<double>(v); }
+
+// sums of (x - pivot) and (x - pivot)^2 over one beam; pivot = first element (keeps the variance
+// free of cancellation when the mean is large, e.g. 2048 channels of uint8 around 128)
+template <typename T>
+__global__ void __launch_bounds__(kDetThreads) detect_stats_kernel(const T* __restrict__ out, int ndm, int64_t n,
+                                                                    int64_t stride, int64_t beam_stride,
+                                                                    double* __restrict__ partial)
+{
+    const T* base = out + static_cast<int64_t>(blockIdx.y) * beam_stride;
+    const double pivot = to_f64(base[0]);
+    double s1 = 0.0, s2 = 0.0;
+    const int64_t n4 = n / 4;
+    for (int d = blockIdx.x; d < ndm; d += gridDim.x) {
+        const T* row = base + static_cast<int64_t>(d) * stride;  // 16-byte aligned (stride % 4 == 0)
+        for (int64_t q = threadIdx.x; q < n4; q += kDetThreads) {
+            const int4 raw = *reinterpret_cast<const int4*>(row + 4 * q);
+            const T* v = reinterpret_cast<const T*>(&raw);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double x = to_f64(v[k]) - pivot;
+                s1 += x;
+                s2 += x * x;
+            }
+        }
+        for (int64_t t = 4 * n4 + threadIdx.x; t < n; t += kDetThreads) {
+            const double x = to_f64(row[t]) - pivot;
+            s1 += x;
+            s2 += x * x;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    __shared__ double w1[kDetThreads / 32], w2[kDetThreads / 32];
+    if ((threadIdx.x & 31) == 0) {
+        w1[threadIdx.x >> 5] = s1;
+        w2[threadIdx.x >> 5] = s2;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int k = 0; k < kDetThreads / 32; ++k) {
+            a += w1[k];
+            b += w2[k];
+        }
+        double* p = partial + (static_cast<int64_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 2;
+        p[0] = a;
+        p[1] = b;
+    }
+}
+
+// one block per beam: partials in index order -> mean, sigma (population), threshold; cursor = 0
+template <typename T>
+__global__ void detect_finish_kernel(const T* __restrict__ out, int64_t beam_stride, const double* __restrict__ partial,
+                                     int nblocks, double count, double nsigma, dedisp_detect_result* __restrict__ res)
+{
+    if (threadIdx.x != 0)
+        return;
+    const double* p = partial + static_cast<int64_t>(blockIdx.x) * nblocks * 2;
+    double a = 0.0, b = 0.0;
+    for (int k = 0; k < nblocks; ++k) {
+        a += p[2 * k];
+        b += p[2 * k + 1];
+    }
+    const double pivot = to_f64(out[static_cast<int64_t>(blockIdx.x) * beam_stride]);
+    const double m = a / count;
+    double var = b / count - m * m;
+    var = var > 0.0 ? var : 0.0;
+    dedisp_detect_result r;
+    r.mean = pivot + m;
+    r.sigma = sqrt(var);
+    r.threshold = r.mean + nsigma * r.sigma;
+    r.count = 0;
+    res[blockIdx.x] = r;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kDetThreads) detect_emit_kernel(const T* __restrict__ out, int ndm, int64_t n,
+                                                                   int64_t stride, int64_t beam_stride,
+                                                                   dedisp_detect_result* __restrict__ res,
+                                                                   dedisp_event* __restrict__ events, int64_t capacity)
+{
+    const int beam = blockIdx.y;
+    const T* base = out + static_cast<int64_t>(beam) * beam_stride;
+    const double thr = res[beam].threshold;
+    unsigned long long* cursor = reinterpret_cast<unsigned long long*>(&res[beam].count);
+    dedisp_event* ev = events + static_cast<int64_t>(beam) * capacity;
+    auto emit = [&](int64_t t, int d, T v) {
+        const unsigned long long k = atomicAdd(cursor, 1ull);
+        if (static_cast<int64_t>(k) < capacity) {
+            dedisp_event e;
+            e.t = t;
+            e.dm = d;
+            e.value = static_cast<float>(v);
+            ev[k] = e;
+        }
+    };
+    const int64_t n4 = n / 4;
+    for (int d = blockIdx.x; d < ndm; d += gridDim.x) {
+        const T* row = base + static_cast<int64_t>(d) * stride;
+        for (int64_t q = threadIdx.x; q < n4; q += kDetThreads) {
+            const int4 raw = *reinterpret_cast<const int4*>(row + 4 * q);
+            const T* v = reinterpret_cast<const T*>(&raw);
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                if (to_f64(v[k]) > thr)
+                    emit(4 * q + k, d, v[k]);
+        }
+        for (int64_t t = 4 * n4 + threadIdx.x; t < n; t += kDetThreads)
+            if (to_f64(row[t]) > thr)
+                emit(t, d, row[t]);
+    }
+}
+
+template <typename T>
+int launch_detect_t(const void* out, int nbeams, int ndm, int64_t n, int64_t stride, double nsigma,
+                    dedisp_event* events, int64_t capacity, dedisp_detect_result* res, double* partial, int nblocks,
+                    cudaStream_t st, int* launches)
+{
+    const T* o = static_cast<const T*>(out);
+    const int64_t beam_stride = stride * ndm;
+    dim3 grid(nblocks, nbeams);
+    detect_stats_kernel<T><<<grid, kDetThreads, 0, st>>>(o, ndm, n, stride, beam_stride, partial);
+    detect_finish_kernel<T><<<nbeams, 32, 0, st>>>(o, beam_stride, partial, nblocks, static_cast<double>(ndm) * n, nsigma, res);
+    detect_emit_kernel<T><<<grid, kDetThreads, 0, st>>>(o, ndm, n, stride, beam_stride, res, events, capacity);
+    *launches += 3;
+    return static_cast<int>(cudaGetLastError());
+}
+
+}  // namespace
+
+int detect_blocks(int ndm) { return ndm < 1184 ? ndm : 1184; }  // 8 blocks per SM on 148 SMs, whole rows each
+
+int launch_detect(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64_t stride, double nsigma,
+                  dedisp_event* events, int64_t capacity, dedisp_detect_result* res, double* partial, void* stream,
+                  int* launches)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int nb = detect_blocks(ndm);
+    if (t == Elem::F32)
+        return launch_detect_t<float>(out, nbeams, ndm, n, stride, nsigma, events, capacity, res, partial, nb, st, launches);
+    return launch_detect_t<int32_t>(out, nbeams, ndm, n, stride, nsigma, events, capacity, res, partial, nb, st, launches);
+}
+
+}  // namespace dedisp

@@ -169,6 +169,37 @@ def test_random_plans_all_kernels(oracle, seed):
     assert tried >= 4
 
 
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_detect_matches_oracle(oracle, dtype):
+    """dedisp_plan_detect on the GPU's own de-dispersed buffer against oracle.detect on the same
+    buffer: mean, sigma, threshold to 1e-12 relative, the event SET exact (order is
+    free), intensities bit-equal; two beams; a capacity smaller than the count keeps counting."""
+    cf = small_cfg(dtype, nchans=64, ndm=37, n_out=2000 + 3, step=0.4)
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    out = plan.execute(to_dev(x), cf.n_out)
+    host = out.cpu().numpy()
+    for nsig, cap in ((3.0, 1 << 16), (2.0, 50)):
+        results, events = plan.detect(out, nsig, capacity=cap)
+        for b in range(2):
+            mu, sg, thr, ev, val = oracle.detect(host[b], nsig)
+            r = results[b]
+            assert abs(r["mean"] - mu) <= 1e-12 * max(1.0, abs(mu)) and abs(r["sigma"] - sg) <= 1e-11 * sg
+            assert abs(r["threshold"] - thr) <= 1e-11 * abs(thr)
+            assert r["count"] == len(ev) > 0
+            got = events[b]
+            if len(ev) <= cap:
+                order = np.lexsort((got["t"], got["dm"]))
+                assert (np.stack([got["t"][order], got["dm"][order]], axis=1) == ev).all()
+                assert (got["value"][order] == val.astype(np.float32)).all()
+            else:
+                assert len(got) == cap
+                allowed = set(map(tuple, ev.tolist()))
+                assert all((int(t), int(d)) in allowed for t, d in zip(got["t"], got["dm"]))
+    with pytest.raises(dd.DedispError):
+        plan.detect(out[:, :, 1:], 3.0)            # misaligned view
+
+
 def test_kernel_timing_hook(oracle):
     cf = small_cfg()
     tab, x = make_case(oracle, cf)
