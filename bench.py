@@ -340,6 +340,23 @@ def main():
            "peak_gbs": pk["hbm_gbs"], "frac": (in_bytes + out_bytes) / (ms_step * 1e-3) / 1e9 / pk["hbm_gbs"],
            "peak_src": pk["src"]}
 
+    # ---- event detection on the step's output: HBM-bound, two
+    # passes over out (statistics, threshold scan); timed on its own, not part of the step
+    plan.detect(out, 5.0, capacity=1 << 16)
+    d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    d0.record()
+    for _ in range(5):
+        dres, _ev = plan.detect(out, 5.0, capacity=1 << 16)
+    d1.record()
+    torch.cuda.synchronize()
+    det_ms = d0.elapsed_time(d1) / 5
+    det_bytes = 2.0 * float(nb) * cf.ndm * n_out * 4
+    detect = {"nsigma": 5.0, "ms": det_ms, "events": [r["count"] for r in dres], "algorithmic_bytes": det_bytes,
+              "achieved_gbs": det_bytes / (det_ms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
+              "frac": det_bytes / (det_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
+              "note": "includes the host read-back of 32 bytes of statistics per beam and of the stored events"}
+
     cpu = None
     if not args.no_cpu_baseline:
         run, sadds, desc, cores = oracle_sample(cf)
@@ -361,7 +378,7 @@ def main():
                        "l2": "inputs larger than L2 (%.2f GB in, %.2f GB out per step)" % (in_bytes / 1e9, out_bytes / 1e9),
                        "parallelism": "1 beam per GPU, no collective" if world > 1 else "single GPU"},
             "real_time_factor": n_out * cf.t_samp_ms * 1e-3 / (ms_step * 1e-3),
-            "roofline": roof, "subband": subband, "hbm": hbm, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roof, "subband": subband, "hbm": hbm, "detect": detect, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
             "paper_context": "paper: 50-200x over one Xeon 2.7 GHz core on a Tesla C1060 (PAPER.md:203), ~1.5e10 adds/s",
             "input_gen_s": t_gen}
