@@ -109,6 +109,7 @@ struct WindowArgs {
     const int32_t* theta;
     int64_t in_stride, out_stride, pair_stride, in_len, n_out;
     int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t, nband, stage_total, theta_max;
+    int flush_rows;  // rows per transpose pass of the flush (set by the launcher)
     int dm_group;  // DM tiles per block-order group (kernels_window.cu)
     const int32_t* band;    // HOST pointer, [nband + 1]
     const int32_t* stage0;  // HOST pointer, [nband + 1]

@@ -19,7 +19,6 @@
 //     accumulators go through a per-warp shared-memory transpose to coalesced global accesses:
 //     band 0 stores, later bands add to what is there.
 #include <cuda_runtime.h>
-#include <cstdlib>
 
 #include "dedisp_internal.h"
 
@@ -366,8 +365,12 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     }
 
     // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
+    // The rows go through a shared-memory transpose (overlaying the ring) in passes of `rpp` rows with
+    // their own regions: all rows of a pass are written, ONE __syncwarp, then read back and stored.
+    // (A sync per row waits for the previous row's global stores every time: 3.5 % of the kernel.)
     asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");  // consumers only: the ring is free now
-    u64* tr = reinterpret_cast<u64*>(smem + tr_off) + warp * W;
+    const int rpp = a.flush_rows;
+    u64* tr = reinterpret_cast<u64*>(smem + tr_off) + static_cast<size_t>(warp) * rpp * W;
     const bool first = band == 0;
     OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
     const int H = a.H;
@@ -375,22 +378,29 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     const int64_t tw = T0 + wt * H;
     // every sample of this warp's two output ranges inside [0, n_out): no bounds tests
     const bool inside = tw - a.theta_max >= 0 && tw + hp + H <= a.n_out;
+    int pass0 = 0;  // first row of the current pass
 #pragma unroll
     for (int j = 0; j < D; ++j) {
-        const int d = ty * RB + g * D + j;
-        const int kf = __shfl_sync(0xffffffffu, kf_lane, j), th = __shfl_sync(0xffffffffu, th_lane, j);
-        __syncwarp();
+        u64* trj = tr + (j - pass0) * W;
 #pragma unroll
         for (int i = 0; i < T; ++i)
-            tr[lane_pinned * T + i] = acc[j][i];
+            trj[lane_pinned * T + i] = acc[j][i];
+        if (j + 1 - pass0 < rpp && j + 1 < D)
+            continue;
         __syncwarp();
-        if (d < a.ndm) {
+#pragma unroll 1
+        for (int jj = pass0; jj <= j; ++jj) {
+            const int d = ty * RB + g * D + jj;
+            const int kf = __shfl_sync(0xffffffffu, kf_lane, jj), th = __shfl_sync(0xffffffffu, th_lane, jj);
+            if (d >= a.ndm)
+                continue;
+            const u64* trr = tr + (jj - pass0) * W + kf;
             OutT* o = out + static_cast<int64_t>(d) * a.out_stride + (tw - th);
             u64 v[T];
 #pragma unroll
             for (int k = 0; k < T; ++k) {
                 const int q = lane_pinned + 32 * k;
-                v[k] = q < H ? tr[q + kf] : 0ull;
+                v[k] = q < H ? trr[q] : 0ull;
             }
             if (inside) {
 #pragma unroll
@@ -413,6 +423,9 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
                 }
             }
         }
+        pass0 = j + 1;
+        if (j + 1 < D)
+            __syncwarp();  // the regions are rewritten by the next pass
     }
 }
 
@@ -449,17 +462,18 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     if (nst == 0)
         return static_cast<int>(cudaErrorInvalidConfiguration);
     const int stages_off = (16 * nst + 127) & ~127;
-    size_t smem = static_cast<size_t>(stages_off) +
-                  static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
-    if (const char* e = getenv("DEDISP_EXP_SMEM_PAD"))
-        smem += atoi(e);
+    const size_t ring = static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
+    const size_t smem = static_cast<size_t>(stages_off) + ring;
+    WindowArgs a2 = a;  // rows per flush pass: as many [NCW][W] u64 transposes as the ring holds
+    a2.flush_rows = static_cast<int>(ring / (static_cast<size_t>(G) * NT * 32 * T * 8));
+    a2.flush_rows = a2.flush_rows > D ? D : a2.flush_rows < 1 ? 1 : a2.flush_rows;
     cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, D, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
         return static_cast<int>(e);
     dim3 grid(static_cast<unsigned>(a.ntile_dm) * a.ntile_t, 1, a.nbeams);
     for (int b = 0; b < a.nband; ++b) {
-        window_kernel<T, G, NT, D, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a, a.band[b], a.band[b + 1], b,
+        window_kernel<T, G, NT, D, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a2, a.band[b], a.band[b + 1], b,
                                                                               a.stage0[b], nst, slot_bytes);
         ++*launches;
         e = cudaGetLastError();
