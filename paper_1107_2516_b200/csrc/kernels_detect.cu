@@ -3,7 +3,7 @@
 // (time, DM trial, intensity) triplet.  HBM-bound: two passes over out[ndm][n] (statistics, then the
 // threshold scan), 16-byte loads, fp64 sums reduced in a fixed order (per-thread, warp shuffles,
 // per-block partials, one finishing block), so mu, sigma and therefore the event set do not depend
-// on scheduling; only the ORDER of the triplets does (an atomic cursor).
+// on scheduling; only the ORDER of the triplets does (an atomic cursor, advanced once per warp and test).
 #include <cuda_runtime.h>
 
 #include "dedisp_internal.h"
@@ -104,8 +104,15 @@ __global__ void __launch_bounds__(kDetThreads) detect_emit_kernel(const T* __res
     const double thr = res[beam].threshold;
     unsigned long long* cursor = reinterpret_cast<unsigned long long*>(&res[beam].count);
     dedisp_event* ev = events + static_cast<int64_t>(beam) * capacity;
+    // one atomic per warp and test: the lanes that found an event take consecutive slots
+    const unsigned lane = threadIdx.x & 31;
     auto emit = [&](int64_t t, int d, T v) {
-        const unsigned long long k = atomicAdd(cursor, 1ull);
+        const unsigned act = __activemask();
+        const int leader = __ffs(act) - 1;
+        unsigned long long k = 0;
+        if (lane == static_cast<unsigned>(leader))
+            k = atomicAdd(cursor, static_cast<unsigned long long>(__popc(act)));
+        k = __shfl_sync(act, k, leader) + __popc(act & ((1u << lane) - 1u));
         if (static_cast<int64_t>(k) < capacity) {
             dedisp_event e;
             e.t = t;
