@@ -278,10 +278,6 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     const int g = uwarp / NT, wt = uwarp % NT;
     int lane_pinned;  // volatile: not rematerialised (S2R) inside the channel loop
     asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane_pinned));
-    // lanes 0..7 fetch the flush parameters of rows 0..7 now, long before they are needed
-    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
-    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
-    const int kf_lane = __ldg(kfp + lane_pinned % D), th_lane = __ldg(thp + lane_pinned % D);
     u64 acc[D][T];
 #pragma unroll
     for (int j = 0; j < D; ++j)
@@ -370,6 +366,9 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // (A sync per row waits for the previous row's global stores every time: 3.5 % of the kernel.)
     asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");  // consumers only: the ring is free now
     const int rpp = a.flush_rows;
+    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
+    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
+    const int kf_lane = __ldg(kfp + lane_pinned % D), th_lane = __ldg(thp + lane_pinned % D);
     u64* tr = reinterpret_cast<u64*>(smem + tr_off) + static_cast<size_t>(warp) * rpp * W;
     const bool first = band == 0;
     OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
@@ -489,12 +488,12 @@ template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_
 #define DEDISP_GEOM(t, gg, nt, dd) \
     if (g.T == t && g.G == gg && g.NT == nt && g.D == dd) \
         return launch_bands<t, gg, nt, dd, OutT>(a, st, launches);
+    DEDISP_GEOM(15, 6, 2, 4)
+    DEDISP_GEOM(15, 4, 3, 4)
     DEDISP_GEOM(21, 4, 1, 4)
     DEDISP_GEOM(21, 8, 1, 4)
-    DEDISP_GEOM(19, 4, 1, 4)
     DEDISP_GEOM(17, 4, 1, 5)
     DEDISP_GEOM(15, 4, 1, 6)
-    DEDISP_GEOM(11, 4, 1, 8)
     DEDISP_GEOM(11, 8, 1, 8)
 #undef DEDISP_GEOM
     return static_cast<int>(cudaErrorInvalidConfiguration);

@@ -27,11 +27,13 @@ namespace dedisp {
 WindowGeom window_default_geom()
 {
     WindowGeom g;
-    // 4 rows x 21 pairs per thread, 4 row groups per block, two blocks per SM: fewer row variants
-    // (branches) per add than 8 x 11 and a slower drift between a thread's rows, so fewer bands
-    g.T = 21;
-    g.G = 4;
-    g.NT = 1;
+    // 4 rows x 15 pairs per thread, 6 row groups x 2 warps along time = 12 consumer warps (three per
+    // scheduler, 160 registers each) in one block per SM.  4 rows instead of 8: fewer row variants
+    // (branches) per add and a slower drift between a thread's rows, so fewer bands.  4 x 21 pairs with
+    // 8 consumer warps (21,4,1,4) is within 2 % (better on cfg 2, worse on cfg 3 and cfg 5).
+    g.T = 15;
+    g.G = 6;
+    g.NT = 2;
     g.D = 4;
     // development override: DEDISP_WINDOW_GEOM="T,G,NT[,D]" (one of the instantiated geometries)
     if (const char* e = std::getenv("DEDISP_WINDOW_GEOM")) {
