@@ -107,11 +107,11 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
-__device__ __forceinline__ u64 add2(u64 a, u64 b)
+// in place (tied operand): with a separate destination ptxas adds into a fresh register pair and
+// copies it back when registers are short (4 IMAD.MOV per channel at 160 registers)
+__device__ __forceinline__ void add2(u64& a, u64 b)
 {
-    u64 r;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
+    asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(b));
 }
 
 #include "window_rows.inc"
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     auto adds = [&](u64(&w)[T + 1], unsigned m) {
 #pragma unroll
         for (int k = 0; k < T; ++k)
-            acc[0][k] = add2(acc[0][k], w[k]);
+            add2(acc[0][k], w[k]);
         rows7(acc, w, m);
     };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
