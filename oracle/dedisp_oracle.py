@@ -126,6 +126,31 @@ def brute_samples(x, shift, d_idx, t_idx):
     return out, sa
 
 
+def subband_sample_indices(tab, d_idx, t_idx):
+    """For single outputs of the two-stage method: the input sample each channel
+    contributes, idx[i][c] = t_i + s2[d_i][sub(c)] + s1[k(d_i)][c] (stage 2 reads the partial series
+    of subband sub(c) at t + s2, which stage 1 formed from channel c at that time + s1).  The caller
+    gathers x[c][idx[i][c]] (from wherever the input lives) and sums in fp64: `sum_samples`.
+    Pinned by equality with `subband` on the small P8 cases."""
+    nchans = tab.s1.shape[1]
+    cps = nchans // tab.s2.shape[1]
+    sub = np.arange(nchans) // cps
+    d = np.asarray(d_idx, dtype=np.int64)
+    k = d // tab.nfine
+    return (np.asarray(t_idx, dtype=np.int64)[:, None] + tab.s2[d][:, sub].astype(np.int64)
+            + tab.s1[k].astype(np.int64))
+
+
+def sum_samples(vals):
+    """fp64 (int64 for integer input) sum over the channel axis and sum of magnitudes."""
+    v = np.asarray(vals)
+    if np.issubdtype(v.dtype, np.integer):
+        s = v.astype(np.int64).sum(axis=1)
+        return s, s.astype(np.float64)
+    v = v.astype(np.float64)
+    return v.sum(axis=1), np.abs(v).sum(axis=1)
+
+
 class SubbandTables:
     pass
 

@@ -377,3 +377,71 @@ def test_cfg3_full_size_sampled(oracle):
     row0 = out[0].cpu().numpy().astype(np.float64)
     s0 = x[:, :cf.n_out].sum(axis=0, dtype=np.float64)
     assert np.abs(row0 - s0).max() <= 1e-5 * np.abs(x[:, :cf.n_out]).sum(axis=0, dtype=np.float64).max()
+
+
+def test_cfg2_full_size_every_output(oracle):
+    """BASELINE cfg 2 at full size (1024 ch x 2048 trials x 65536 samples, two channel bands in the
+    window kernel): every output against the oracle."""
+    cf = synth.configs()[2]
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    pulses = synth.draw_pulses(cf, cf.n_out)
+    x = synth.make_input(cf, cf.n_out + int(tab.max()), pulses, {p[0]: tab[p[0]] for p in pulses})
+    plan = dd.Plan(**cf.plan_args())
+    got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+    for r0 in range(0, cf.ndm, 512):                       # the oracle in slabs of 512 trials (memory)
+        ref, sa = oracle.brute_f32(x, tab[r0:r0 + 512], cf.n_out)
+        check_f32(got[r0:r0 + 512], ref, sa)
+
+
+def test_cfg4_full_size_sampled(oracle):
+    """BASELINE cfg 4 at full size in bench.py's launch configuration (9.1 GB of input generated on the
+    device, long-tile kernel for both stages): 200 outputs over the (DM, time) plane recomputed one by
+    one from the oracle's own subband tables; the gather of the 4096 contributing input samples per
+    output is plain indexing on the device tensor, the fp64 sums are the oracle's."""
+    cf = synth.configs()[4]
+    tab = oracle.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list, cf.nsub, cf.nfine)
+    plan = dd.Plan(**cf.plan_args())
+    assert plan.max_delay == tab.max_delay
+    n_in = cf.n_out + tab.max_delay
+    stride = (n_in + 15) // 16 * 16
+    g = torch.Generator(device="cuda").manual_seed(cf.seed)
+    x = torch.empty((cf.nchans, stride), dtype=torch.float32, device="cuda")
+    for c0 in range(0, cf.nchans, 256):
+        x[c0:c0 + 256].normal_(generator=g)
+    out = plan.execute(x[:, :n_in], cf.n_out)
+    rng = np.random.default_rng(4)
+    d = np.r_[rng.integers(0, cf.ndm, 180), [0, 16, cf.ndm - 1, cf.ndm - 32] * 5]
+    t = np.r_[rng.integers(0, cf.n_out, 180), [0, cf.n_out - 1] * 10]
+    idx = oracle.subband_sample_indices(tab, d, t)
+    assert idx.max() < n_in
+    cc = torch.arange(cf.nchans, device="cuda")[None, :].expand(len(d), -1)
+    vals = x[cc, torch.from_numpy(idx).cuda()].cpu().numpy()
+    ref, sa = oracle.sum_samples(vals)
+    got = out[torch.from_numpy(d).cuda(), torch.from_numpy(t).cuda()].cpu().numpy()
+    check_f32(got, ref, sa)
+    del x, out
+    torch.cuda.empty_cache()
+
+
+def test_cfg5_full_size_streaming_sampled(oracle):
+    """BASELINE cfg 5 at full chunk size (4 beams x 2048 ch x 65536-sample chunks, 3072 trials, uint8):
+    two pushes through the streaming driver; 400 outputs of the second push (which reach back into the
+    first chunk through the carry) recomputed one by one, bit-exact."""
+    cf = synth.configs()[5]
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    M, C, nb = int(tab.max()), cf.n_out, cf.nbeams
+    xs = np.stack([synth.make_input(cf, 2 * C, beam=b) for b in range(nb)])
+    plan = dd.Plan(**cf.plan_args())
+    st = dd.Stream(plan, dd.U8, C, nb)
+    out = torch.empty((nb, cf.ndm, C), dtype=torch.int32, device="cuda")
+    st.push(torch.from_numpy(np.ascontiguousarray(xs[:, :, :C])).cuda(), out)
+    st.push(torch.from_numpy(np.ascontiguousarray(xs[:, :, C:])).cuda(), out)
+    rng = np.random.default_rng(5)
+    d = np.r_[rng.integers(0, cf.ndm, 380), [0, cf.ndm - 1] * 10]
+    tl = np.r_[rng.integers(0, C, 380), [0, C - 1, 0, C - 1] * 5]      # time inside the second push's output
+    for b in range(nb):
+        ref, _ = oracle.brute_samples(xs[b], tab, d, tl + C - M)       # stream time of output tl of push 1
+        got = out[b][torch.from_numpy(d).cuda(), torch.from_numpy(tl).cuda()].cpu().numpy()
+        assert (got == ref).all()
+    st.close()
+    plan.close()

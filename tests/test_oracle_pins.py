@@ -406,3 +406,14 @@ def test_detect_paper_fig5_statement(oracle):
     on = ((ev[:, 0] >= 500) & (ev[:, 0] < 500 + w)) | ((ev[:, 0] >= 1500) & (ev[:, 0] < 1500 + w))
     assert (ev[on, 1] == 5).mean() > 0.9 and on.mean() > 0.95   # at the true trial, inside the pulses
     assert (val > thr).all()
+
+
+def test_subband_sample_indices_equal_the_two_stage_oracle(oracle):
+    """The per-sample form of the two-stage sum (used to spot-check full-size GPU runs) against the
+    stage-by-stage oracle on every output of a small case, uint8 so that equality is exact."""
+    cf, full, tab, x = _sub_case(oracle, nsub=4, dtype="u8", n_out=123)
+    ref, _ = oracle.subband(x, tab, cf.n_out)
+    d, t = np.divmod(np.arange(cf.ndm * cf.n_out), cf.n_out)
+    idx = oracle.subband_sample_indices(tab, d, t)
+    got, sa = oracle.sum_samples(x[np.arange(cf.nchans)[None, :], idx])
+    assert (got.reshape(cf.ndm, cf.n_out) == ref).all() and (sa == got).all()
