@@ -307,14 +307,17 @@ def main():
     subband = None
     if cf.nsub:
         # the two-stage path executes far fewer adds than the brute-force-equivalent count `value`
-        # is quoted in: stage 1 = sum_k (n_out + maxshift2_k) * nchans, stage 2 = ndm * n_out * nsub.
+        # is quoted in: stage 1 = sum_{k,s} (n_out + maxshift2_{k,s}) * nchans/nsub, stage 2 = ndm * n_out * nsub.
         # Stage 1 (the dominant kernel) has no reuse between rows: one shared-memory word per add,
         # so its ceiling is the 128 B/clk/SM shared-memory pipe = a quarter of the add pipe.
-        m2 = plan.subband_shifts()[3].astype(np.float64)
-        s1_adds = float(nb) * float((n_out + m2).sum()) * cf.nchans
+        # stage 1 forms n_out + max_{d in group k} s2(d, s) samples of subband s in group k (what stage 2 reads)
+        s2tab = plan.subband_shifts()[1].astype(np.float64)
+        mks = s2tab.reshape(cf.ndm // cf.nfine, cf.nfine, cf.nsub).max(axis=1)          # [ncoarse][nsub]
+        s1_samples = float((n_out + mks).sum())                                          # per channel of a subband
+        s1_adds = float(nb) * s1_samples * (cf.nchans // cf.nsub)
         s2_adds = float(nb) * cf.ndm * float(n_out) * cf.nsub
         s1_ms, s2_ms = (float(np.mean([v[k] for v in sms])) for k in (0, 1))
-        s2_bytes = float(nb) * (float((n_out + m2).sum()) * cf.nsub * 4 + float(cf.ndm) * n_out * 4)
+        s2_bytes = float(nb) * (s1_samples * 4 + float(cf.ndm) * n_out * 4)
         smem_peak = nsm * 32 * pk["sm_max_mhz"] * 1e6
         kernel_adds, kernel_ms_dom = s1_adds, s1_ms
         kname = "%s (subband stage 1)" % kname

@@ -74,13 +74,14 @@ struct dedisp_plan {
     int spread_full[3] = {0, 0, 0};
     // subband
     std::vector<int32_t> s1, s2, maxshift2;
+    std::vector<int32_t> maxshift2_ks;  // [nsub][ncoarse]: what stage 2 reads of subband s in group k
     std::vector<double> nominal;
     int32_t maxshift2_max = 0;
     int spread_s1[3] = {0, 0, 0}, spread_s2[3] = {0, 0, 0};
     // device side (uploaded by the first execute)
     bool uploaded = false;
     int device = -1;
-    int32_t *d_shift = nullptr, *d_s1 = nullptr, *d_s2 = nullptr, *d_maxshift2 = nullptr;
+    int32_t *d_shift = nullptr, *d_s1 = nullptr, *d_s2 = nullptr, *d_maxshift2 = nullptr, *d_maxshift2_ks = nullptr;
     DevBuf scratch;            // subband intermediate
     DevBuf host_in, host_out;  // staging for dedisp_execute_host
     DevBuf det_partial;        // dedisp_plan_detect workspace
@@ -157,6 +158,8 @@ dedisp_status upload(dedisp_plan* p)
             e = up(&p->d_s2, p->s2);
         if (e == cudaSuccess)
             e = up(&p->d_maxshift2, p->maxshift2);
+        if (e == cudaSuccess)
+            e = up(&p->d_maxshift2_ks, p->maxshift2_ks);
     }
     if (e != cudaSuccess) {
         cudaGetLastError();
@@ -333,7 +336,9 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     pr.in = in;
     pr.out = plan->scratch.p;
     pr.shift = plan->d_s1;
-    pr.row_extra = plan->d_maxshift2;
+    // stage 1 forms, for subband s of group k, only the samples stage 2 reads: n_out + max_d s2(d, s)
+    pr.row_extra = plan->d_maxshift2_ks;
+    pr.row_extra_b1_stride = ncoarse;
     pr.in_chan_stride = in_stride;
     pr.in_b0_stride = in_stride * plan->nchans;
     pr.in_b1_stride = in_stride * cps;
@@ -447,6 +452,13 @@ dedisp_status dedisp_plan_create(dedisp_plan** plan, int nchans, double f_top_mh
             const int ncoarse = ndm / nfine;
             for (int k = 0; k < ncoarse; ++k)
                 p->maxshift2_max = p->maxshift2[k] > p->maxshift2_max ? p->maxshift2[k] : p->maxshift2_max;
+            p->maxshift2_ks.assign(static_cast<size_t>(nsub) * ncoarse, 0);
+            for (int d = 0; d < ndm; ++d)
+                for (int s = 0; s < nsub; ++s) {
+                    int32_t& m = p->maxshift2_ks[static_cast<size_t>(s) * ncoarse + d / nfine];
+                    const int32_t v = p->s2[static_cast<size_t>(d) * nsub + s];
+                    m = v > m ? v : m;
+                }
             for (int k = 0; k < 3; ++k) {
                 p->spread_s1[k] = tile_spread(p->s1.data(), ncoarse, nchans, nchans, tiles[k]);
                 int w = 0;
@@ -477,6 +489,7 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         cudaFree(p->d_s1);
         cudaFree(p->d_s2);
         cudaFree(p->d_maxshift2);
+        cudaFree(p->d_maxshift2_ks);
         cudaFree(p->d_win_meta);
         cudaFree(p->d_win_kfinal);
         cudaFree(p->d_win_theta);

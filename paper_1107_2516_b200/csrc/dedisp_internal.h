@@ -25,7 +25,8 @@ struct Problem {
     const void* in;
     void* out;
     const int32_t* shift;    // device
-    const int32_t* row_extra;  // device [ndm] or nullptr: row d has n_base + row_extra[d] outputs
+    const int32_t* row_extra;  // device [nb1][ndm] or nullptr: row (b1, d) has n_base + row_extra[b1][d] outputs
+    int64_t row_extra_b1_stride;
     int64_t in_chan_stride, in_b0_stride, in_b1_stride;
     int64_t in_len;  // samples that may be read from one channel row
     int64_t out_dm_stride, out_b0_stride, out_b1_stride;

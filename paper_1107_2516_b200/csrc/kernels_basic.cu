@@ -24,7 +24,7 @@ __global__ void __launch_bounds__(256) naive_kernel(Problem p)
     const int64_t t = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
     const int d = blockIdx.y;
     const int b1 = blockIdx.z % p.nb1, b0 = blockIdx.z / p.nb1;
-    const int64_t len = p.row_extra ? p.n_base + p.row_extra[d] : p.n_out;
+    const int64_t len = p.row_extra ? p.n_base + p.row_extra[b1 * p.row_extra_b1_stride + d] : p.n_out;
     if (t >= len)
         return;
     const InT* in = static_cast<const InT*>(p.in) + b0 * p.in_b0_stride + b1 * p.in_b1_stride;
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(kDirectThreads) direct_kernel(Problem p, int c
     // rows of this tile that exist, and the longest of them: a tile beyond every row's length exits
     int64_t tile_len = 0;
     for (int j = 0; j < DBLK && d0 + j < p.ndm; ++j) {
-        const int64_t l = p.row_extra ? p.n_base + p.row_extra[d0 + j] : p.n_out;
+        const int64_t l = p.row_extra ? p.n_base + p.row_extra[b1 * p.row_extra_b1_stride + d0 + j] : p.n_out;
         tile_len = l > tile_len ? l : tile_len;
     }
     if (t0 >= tile_len)
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(kDirectThreads) direct_kernel(Problem p, int c
         const int d = d0 + warp * DT + j;
         if (d >= p.ndm)
             continue;
-        const int64_t len = p.row_extra ? p.n_base + p.row_extra[d] : p.n_out;
+        const int64_t len = p.row_extra ? p.n_base + p.row_extra[b1 * p.row_extra_b1_stride + d] : p.n_out;
         AccT* o = out + static_cast<int64_t>(d) * p.out_dm_stride;
 #pragma unroll
         for (int i = 0; i < kTT; ++i) {

@@ -84,7 +84,7 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) long_kernel(const Problem p, 
 #pragma unroll
     for (int j = 0; j < R; ++j) {
         if (d0 + j < p.ndm) {
-            const int64_t len = p.row_extra ? p.n_base + p.row_extra[d0 + j] : p.n_out;
+            const int64_t len = p.row_extra ? p.n_base + p.row_extra[b1 * p.row_extra_b1_stride + d0 + j] : p.n_out;
             if (t0 < len)
                 act |= 1u << j;
         }
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) long_kernel(const Problem p, 
     }
 
     const int d = d0 + warp;
-    const int64_t len = p.row_extra ? p.n_base + p.row_extra[d] : p.n_out;
+    const int64_t len = p.row_extra ? p.n_base + p.row_extra[b1 * p.row_extra_b1_stride + d] : p.n_out;
     AccT* o = static_cast<AccT*>(p.out) + b0 * p.out_b0_stride + b1 * p.out_b1_stride +
               static_cast<int64_t>(d) * p.out_dm_stride + t0 + lane;
     if (t0 + L <= len && !p.accumulate) {
