@@ -151,8 +151,10 @@ DEDISP_API int64_t dedisp_plan_scratch_bytes(const dedisp_plan *plan, int64_t ns
  *   nsamp_out   output samples per DM trial (>= 0; 0 is a no-op)
  *   cuda_stream a cudaStream_t (NULL = the legacy default stream)
  *
- * Brute-force plans: one kernel.  Subband plans: stage 1 into the plan's scratch (grown on
- * demand, so one execute per plan may be in flight), then stage 2.  Input elements beyond
+ * Brute-force plans: the register-window kernel (a pair-forming pre-pass into plan-owned scratch,
+ * then one launch per channel band) or one long-tile / direct launch.  Subband plans: stage 1
+ * into the plan's scratch (grown on demand, so one execute per plan may be in flight), then
+ * stage 2; stage 1 forms of every (group, subband) series only the samples stage 2 reads.  Input elements beyond
  * nsamp_out + max_delay in a row are never read; output elements beyond nsamp_out in a row are
  * never written.  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ENOMEM, DEDISP_ECUDA.
  */
@@ -162,9 +164,12 @@ DEDISP_API dedisp_status dedisp_execute(dedisp_plan *plan, const void *in, void 
 
 /*
  * Host-buffer convenience: same operation with HOST in/out ([nbeams][nchans][nsamp_out+max_delay]
- * dense input, [nbeams][ndm][nsamp_out] dense output).  Allocates device buffers, copies in,
- * executes, copies out and synchronises the stream.  This is the "end-to-end" entry bench.py
- * times; every arithmetic step still runs in the CUDA kernels.
+ * dense input, [nbeams][ndm][nsamp_out] dense output).  Allocates device buffers (kept by the
+ * plan), copies in, executes, copies out and synchronises the stream.  Brute-force plans with
+ * nsamp_out >= 65536 are cut into up to 8 time pieces whose H2D copy, kernels and D2H copy overlap
+ * on two plan-owned copy streams (pinned host memory is needed for the overlap, not for
+ * correctness).  This is the "end-to-end" entry bench.py times; every arithmetic step still runs
+ * in the CUDA kernels.
  */
 DEDISP_API dedisp_status dedisp_execute_host(dedisp_plan *plan, const void *host_in, void *host_out,
                                   dedisp_dtype dtype, int64_t nsamp_out, int nbeams,
@@ -186,7 +191,8 @@ DEDISP_API dedisp_status dedisp_stream_create(dedisp_stream **s, dedisp_plan *pl
                                    int64_t chunk, int nbeams);
 DEDISP_API dedisp_status dedisp_stream_push(dedisp_stream *s, const void *chunk_in, void *out,
                                  void *cuda_stream);
-/* Same with HOST chunk_in/out (pinned or pageable): H2D copy, push, D2H copy, synchronise. */
+/* Same with HOST chunk_in/out (pinned or pageable): the chunk is copied straight behind the carry
+ * in up to 8 time pieces whose H2D copy, kernels and D2H copy overlap; synchronises the stream. */
 DEDISP_API dedisp_status dedisp_stream_push_host(dedisp_stream *s, const void *host_chunk_in, void *host_out,
                                       void *cuda_stream);
 /* Resets the carry to zeros (asynchronously on cuda_stream). */
