@@ -234,3 +234,18 @@ def detect(out, nsigma):
     thr = mu + float(nsigma) * sigma
     d, t = np.nonzero(x > thr)
     return mu, sigma, thr, np.stack([t, d], axis=1).astype(np.int64), np.asarray(out)[d, t]
+
+
+def power_corner_turn(volt):
+    """Total power of complex voltages, transposed into channel order (steps (iii) and
+    (iv) of the real-time pipeline): out[c][t] = re(volt[t][c])^2 + im(volt[t][c])^2.  The paper's
+    arithmetic is fp32, so the result is DEFINED in fp32 with each product and the sum rounded on its
+    own (reading R15); numpy float32 operations round exactly that way.  Also returns the fp64 value.
+    Pins: exactly representable hand values ((3,4) -> 25, (0.5,-0.25) -> 0.3125), the layout
+    (out[c][t] comes from volt[t][c]), agreement of the fp32 definition with fp64 within 2 ulp."""
+    v = np.asarray(volt)
+    re = v.real.astype(np.float32)
+    im = v.imag.astype(np.float32)
+    p32 = (re * re + im * im).astype(np.float32).T.copy()
+    p64 = (re.astype(np.float64) ** 2 + im.astype(np.float64) ** 2).T.copy()
+    return p32, p64

@@ -417,3 +417,17 @@ def test_subband_sample_indices_equal_the_two_stage_oracle(oracle):
     idx = oracle.subband_sample_indices(tab, d, t)
     got, sa = oracle.sum_samples(x[np.arange(cf.nchans)[None, :], idx])
     assert (got.reshape(cf.ndm, cf.n_out) == ref).all() and (sa == got).all()
+
+
+def test_power_corner_turn_pins(oracle):
+    v = np.zeros((3, 2), dtype=np.complex64)                 # [t][c]
+    v[0, 0], v[1, 0], v[2, 1], v[0, 1] = 3 + 4j, 0.5 - 0.25j, -2j, 1e-3 + 0j
+    p32, p64 = oracle.power_corner_turn(v)
+    assert p32.shape == (2, 3) and p32.dtype == np.float32
+    assert p32[0].tolist() == [25.0, 0.3125, 0.0] and p32[1, 2] == 4.0      # out[c][t] <- volt[t][c]
+    assert p32[1, 0] == np.float32(np.float32(1e-3) * np.float32(1e-3))
+    rng = np.random.default_rng(9)
+    z = (rng.standard_normal((50, 7)) + 1j * rng.standard_normal((50, 7))).astype(np.complex64)
+    p32, p64 = oracle.power_corner_turn(z)
+    assert np.abs(p32 - p64).max() <= 2 * np.spacing(p64.astype(np.float32)).max()
+    assert np.isclose(p64.sum(), np.vdot(z.astype(np.complex128), z.astype(np.complex128)).real)
