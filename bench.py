@@ -360,6 +360,28 @@ def main():
               "frac": det_bytes / (det_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
               "note": "includes the host read-back of 32 bytes of statistics per beam and of the stored events"}
 
+    # ---- power + corner turn: the front-end step that produces the
+    # channel-major layout, on a voltage buffer of up to 2^19 spectra (the paper's buffer) x nchans
+    front = None
+    if cf.dtype == "f32":
+        ns = int(min(n_in, 1 << 19, (1 << 31) // cf.nchans))
+        volt = torch.randn((ns, cf.nchans, 2), dtype=torch.float32, device="cuda")
+        vz = torch.view_as_complex(volt)
+        pw = dd.power_corner_turn(vz)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(5):
+            dd.power_corner_turn(vz, out=pw)
+        f1.record()
+        torch.cuda.synchronize()
+        fms = f0.elapsed_time(f1) / 5
+        fbytes = 12.0 * ns * cf.nchans
+        front = {"op": "power_corner_turn", "spectra": ns, "nchans": cf.nchans, "ms": fms, "algorithmic_bytes": fbytes,
+                 "achieved_gbs": fbytes / (fms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
+                 "frac": fbytes / (fms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm"}
+        del volt, vz, pw
+
     cpu = None
     if not args.no_cpu_baseline:
         run, sadds, desc, cores = oracle_sample(cf)
@@ -381,7 +403,7 @@ def main():
                        "l2": "inputs larger than L2 (%.2f GB in, %.2f GB out per step)" % (in_bytes / 1e9, out_bytes / 1e9),
                        "parallelism": "1 beam per GPU, no collective" if world > 1 else "single GPU"},
             "real_time_factor": n_out * cf.t_samp_ms * 1e-3 / (ms_step * 1e-3),
-            "roofline": roof, "subband": subband, "hbm": hbm, "detect": detect, "cpu_baseline": cpu, "e2e": e2e,
+            "roofline": roof, "subband": subband, "hbm": hbm, "detect": detect, "front_end": front, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
             "paper_context": "paper: 50-200x over one Xeon 2.7 GHz core on a Tesla C1060 (PAPER.md:203), ~1.5e10 adds/s",
             "input_gen_s": t_gen}

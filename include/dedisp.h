@@ -245,6 +245,20 @@ DEDISP_API dedisp_status dedisp_plan_detect(dedisp_plan *plan, const void *out, 
                                             dedisp_event *events, int64_t capacity,
                                             dedisp_detect_result *results, void *cuda_stream);
 
+/*
+ * Power + corner turn, the two steps before de-dispersion in the paper's real-time pipeline
+ * ("(iii) channelizes and calculates total power (iv) transposes data so that it is
+ * in channel order"; Table 6).  One fused kernel:
+ *     out[c][t] = re(volt[t][c])^2 + im(volt[t][c])^2     (fp32, each operation rounded on its own)
+ *   volt   DEVICE, [nsamp][volt_stride] interleaved (re, im) float pairs, spectrum order, one
+ *          polarisation; volt_stride >= nchans (in complex elements); 8-byte aligned
+ *   out    DEVICE, [nchans][out_stride] float, the channel-major layout dedisp_execute reads;
+ *          out_stride >= nsamp
+ * Asynchronous on cuda_stream.  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ECUDA.
+ */
+DEDISP_API dedisp_status dedisp_power_corner_turn(const void *volt, void *out, int nchans, int64_t nsamp,
+                                                  int64_t volt_stride, int64_t out_stride, void *cuda_stream);
+
 /* Static string for a status code. */
 DEDISP_API const char *dedisp_strerror(dedisp_status status);
 

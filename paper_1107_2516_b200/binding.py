@@ -44,6 +44,7 @@ _SIGS = {
     "dedisp_plan_last_kernel_ms": (_int, [_vp, _vp]),
     "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
     "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
+    "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
 }
@@ -235,6 +236,22 @@ class Plan:
         _check(lib().dedisp_execute_host(self._h, xa.ctypes.data, oa.ctypes.data, dt, int(nsamp_out),
                                          int(xa.shape[0]), _stream_ptr(stream)), "dedisp_execute_host")
         return out
+
+
+def power_corner_turn(volt, out=None, stream=None):
+    """dedisp_power_corner_turn: volt CUDA complex64 [nsamp][nchans] (row stride free) -> float32
+    [nchans][nsamp] in the de-disperser's layout (row stride padded to 16 elements)."""
+    import torch
+    if not volt.is_cuda or volt.dtype != torch.complex64 or volt.dim() != 2 or volt.stride(1) != 1:
+        raise DedispError(ESHAPE, "dedisp_power_corner_turn")
+    nsamp, nchans = volt.shape
+    if out is None:
+        stride = (nsamp + 15) // 16 * 16
+        out = torch.empty((nchans, stride), dtype=torch.float32, device=volt.device)[:, :nsamp]
+    _check(lib().dedisp_power_corner_turn(volt.data_ptr(), out.data_ptr(), int(nchans), int(nsamp),
+                                          int(volt.stride(0)), int(out.stride(0)), _stream_ptr(stream)),
+           "dedisp_power_corner_turn")
+    return out
 
 
 class Stream:

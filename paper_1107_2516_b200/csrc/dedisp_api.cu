@@ -944,6 +944,18 @@ dedisp_status dedisp_plan_detect(dedisp_plan* plan, const void* out, dedisp_dtyp
     return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
+dedisp_status dedisp_power_corner_turn(const void* volt, void* out, int nchans, int64_t nsamp, int64_t volt_stride,
+                                       int64_t out_stride, void* cuda_stream)
+{
+    if (!volt || !out || nchans <= 0 || nsamp < 0)
+        return DEDISP_EINVAL;
+    if (volt_stride < nchans || out_stride < nsamp || (reinterpret_cast<uintptr_t>(volt) & 7) != 0 ||
+        (reinterpret_cast<uintptr_t>(out) & 3) != 0)
+        return DEDISP_ESHAPE;
+    return launch_power_corner_turn(volt, out, nchans, nsamp, volt_stride, out_stride, cuda_stream) == 0 ? DEDISP_OK
+                                                                                                         : DEDISP_ECUDA;
+}
+
 const char* dedisp_strerror(dedisp_status s)
 {
     switch (s) {

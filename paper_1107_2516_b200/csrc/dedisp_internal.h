@@ -57,6 +57,10 @@ int launch_detect(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64
                   dedisp_event* events, int64_t capacity, dedisp_detect_result* res, double* partial, void* stream,
                   int* launches);
 
+// kernels_front.cu: out[c][t] = |volt[t][c]|^2, strides in elements
+int launch_power_corner_turn(const void* volt, void* out, int nchans, int64_t nsamp, int64_t volt_stride,
+                             int64_t out_stride, void* stream);
+
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
 // Geometry: a consumer warp owns the D (4 or 8) DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
