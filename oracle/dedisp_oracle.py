@@ -249,3 +249,20 @@ def power_corner_turn(volt):
     p32 = (re * re + im * im).astype(np.float32).T.copy()
     p64 = (re.astype(np.float64) ** 2 + im.astype(np.float64) ** 2).T.copy()
     return p32, p64
+
+
+def bin_samples(x, nb):
+    """Binning, stage (i) of the paper's subband scheme ("Binning averages N_b
+    consecutive samples"): out[c][j] = (x[c][j*nb] + ... + x[c][j*nb + nb-1]) / nb, floor(n/nb)
+    outputs per channel (a ragged tail is dropped).  Reading R16: fp32 like the paper's pipeline, the
+    sum taken left to right and divided once, every operation rounded on its own -- so the result is
+    defined bit for bit; the fp64 value is returned beside it.
+    Pins: nb = 1 is the identity; hand values; constant input stays constant; agreement with the
+    fp64 mean within nb ulp."""
+    x = np.asarray(x, dtype=np.float32)
+    n = x.shape[-1] // nb
+    v = x[..., :n * nb].reshape(x.shape[:-1] + (n, nb))
+    acc = v[..., 0].copy()
+    for i in range(1, nb):
+        acc = (acc + v[..., i]).astype(np.float32)
+    return (acc / np.float32(nb)).astype(np.float32), v.astype(np.float64).mean(axis=-1)

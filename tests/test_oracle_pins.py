@@ -431,3 +431,16 @@ def test_power_corner_turn_pins(oracle):
     p32, p64 = oracle.power_corner_turn(z)
     assert np.abs(p32 - p64).max() <= 2 * np.spacing(p64.astype(np.float32)).max()
     assert np.isclose(p64.sum(), np.vdot(z.astype(np.complex128), z.astype(np.complex128)).real)
+
+
+def test_bin_samples_pins(oracle):
+    x = np.arange(14, dtype=np.float32).reshape(2, 7)
+    assert (oracle.bin_samples(x, 1)[0] == x).all()                               # identity
+    assert oracle.bin_samples(x, 2)[0].tolist() == [[0.5, 2.5, 4.5], [7.5, 9.5, 11.5]]   # tail dropped
+    assert oracle.bin_samples(x, 4)[0].tolist() == [[1.5], [8.5]]
+    assert (oracle.bin_samples(np.full((3, 64), 0.1, np.float32), 4)[0] == np.float32(0.1)).all()
+    g = np.random.default_rng(2).standard_normal((5, 999)).astype(np.float32)
+    for nb in (2, 3, 4, 8):
+        b32, b64 = oracle.bin_samples(g, nb)
+        assert b32.shape == (5, 999 // nb)
+        assert np.abs(b32 - b64).max() <= nb * np.spacing(np.float32(np.abs(g).max()))
