@@ -381,6 +381,20 @@ def main():
                  "achieved_gbs": fbytes / (fms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
                  "frac": fbytes / (fms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm"}
         del volt, vz, pw
+        # binning, bin factor 2 on the step's own input
+        bx = x[0]
+        dd.bin_samples(bx, 2)
+        torch.cuda.synchronize()
+        f0.record()
+        for _ in range(5):
+            dd.bin_samples(bx, 2)
+        f1.record()
+        torch.cuda.synchronize()
+        bms = f0.elapsed_time(f1) / 5
+        bbytes = 6.0 * cf.nchans * float(bx.shape[-1])
+        front["binning"] = {"nb": 2, "ms": bms, "algorithmic_bytes": bbytes, "achieved_gbs": bbytes / (bms * 1e-3) / 1e9,
+                            "frac": bbytes / (bms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
+                            "note": "includes the allocation of the output tensor in the binding"}
 
     cpu = None
     if not args.no_cpu_baseline:

@@ -259,6 +259,19 @@ DEDISP_API dedisp_status dedisp_plan_detect(dedisp_plan *plan, const void *out, 
 DEDISP_API dedisp_status dedisp_power_corner_turn(const void *volt, void *out, int nchans, int64_t nsamp,
                                                   int64_t volt_stride, int64_t out_stride, void *cuda_stream);
 
+/*
+ * Binning, stage (i) of the paper's subband scheme ("Binning averages N_b consecutive
+ * samples"; eq. 6): out[r][j] = (in[r][j*nb] + ... + in[r][j*nb + nb-1]) / nb for j < nsamp / nb
+ * (a ragged tail is dropped), fp32, the sum left to right, every operation rounded on its own.
+ * A survey pass with bin factor b (Table 1) is this call followed by a plan created with
+ * t_samp * b.
+ *   in     DEVICE, [nrows][in_stride] float (nrows = nbeams * nchans); in_stride >= nsamp
+ *   out    DEVICE, [nrows][out_stride] float; out_stride >= nsamp / nb; must not overlap in
+ * Asynchronous on cuda_stream.  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ECUDA.
+ */
+DEDISP_API dedisp_status dedisp_bin(const void *in, void *out, int64_t nrows, int64_t nsamp, int64_t in_stride,
+                                    int64_t out_stride, int nb, void *cuda_stream);
+
 /* Static string for a status code. */
 DEDISP_API const char *dedisp_strerror(dedisp_status status);
 

@@ -45,6 +45,7 @@ _SIGS = {
     "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
     "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
+    "dedisp_bin": (_int, [_vp, _vp, _i64, _i64, _i64, _i64, _int, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
 }
@@ -252,6 +253,27 @@ def power_corner_turn(volt, out=None, stream=None):
                                           int(volt.stride(0)), int(out.stride(0)), _stream_ptr(stream)),
            "dedisp_power_corner_turn")
     return out
+
+
+def bin_samples(x, nb, stream=None):
+    """dedisp_bin: x CUDA float32 [..., n] (last dim contiguous, uniform row stride) -> [..., n // nb]
+    with a row stride padded to 16 elements (ready for dedisp_execute)."""
+    import torch
+    if not x.is_cuda or x.dtype != torch.float32 or x.stride(-1) != 1 or x.dim() < 2:
+        raise DedispError(ESHAPE, "dedisp_bin")
+    rows = 1
+    for k in range(x.dim() - 1):
+        rows *= x.shape[k]
+    for k in range(x.dim() - 2):
+        if x.stride(k) != x.stride(k + 1) * x.shape[k + 1]:
+            raise DedispError(ESHAPE, "dedisp_bin")
+    n = x.shape[-1]
+    nout = n // int(nb)
+    stride = max(16, (nout + 15) // 16 * 16)
+    out = torch.empty(tuple(x.shape[:-1]) + (stride,), dtype=torch.float32, device=x.device)
+    _check(lib().dedisp_bin(x.data_ptr(), out.data_ptr(), int(rows), int(n), int(x.stride(-2)), int(stride),
+                            int(nb), _stream_ptr(stream)), "dedisp_bin")
+    return out[..., :nout]
 
 
 class Stream:

@@ -956,6 +956,16 @@ dedisp_status dedisp_power_corner_turn(const void* volt, void* out, int nchans, 
                                                                                                          : DEDISP_ECUDA;
 }
 
+dedisp_status dedisp_bin(const void* in, void* out, int64_t nrows, int64_t nsamp, int64_t in_stride, int64_t out_stride,
+                         int nb, void* cuda_stream)
+{
+    if (!in || !out || nrows <= 0 || nsamp < 0 || nb <= 0)
+        return DEDISP_EINVAL;
+    if (in_stride < nsamp || out_stride < nsamp / nb)
+        return DEDISP_ESHAPE;
+    return launch_bin(in, out, nrows, nsamp / nb, in_stride, out_stride, nb, cuda_stream) == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
 const char* dedisp_strerror(dedisp_status s)
 {
     switch (s) {

@@ -61,6 +61,9 @@ int launch_detect(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64
 int launch_power_corner_turn(const void* volt, void* out, int nchans, int64_t nsamp, int64_t volt_stride,
                              int64_t out_stride, void* stream);
 
+int launch_bin(const void* in, void* out, int64_t nrows, int64_t nout, int64_t in_stride, int64_t out_stride, int nb,
+               void* stream);
+
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
 // Geometry: a consumer warp owns the D (4 or 8) DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
