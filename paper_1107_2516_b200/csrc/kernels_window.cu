@@ -20,6 +20,8 @@
 //     band 0 stores, later bands add to what is there.
 #include <cuda_runtime.h>
 
+#include <cstdlib>
+
 #include "dedisp_internal.h"
 
 namespace dedisp {
@@ -466,6 +468,8 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     WindowArgs a2 = a;  // rows per flush pass: as many [NCW][W] u64 transposes as the ring holds
     a2.flush_rows = static_cast<int>(ring / (static_cast<size_t>(G) * NT * 32 * T * 8));
     a2.flush_rows = a2.flush_rows > D ? D : a2.flush_rows < 1 ? 1 : a2.flush_rows;
+    if (const char* e = std::getenv("DEDISP_WINDOW_FLUSH_ROWS"))  // development override (fewer rows per pass)
+        a2.flush_rows = std::atoi(e) >= 1 && std::atoi(e) < a2.flush_rows ? std::atoi(e) : a2.flush_rows;
     cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, D, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
