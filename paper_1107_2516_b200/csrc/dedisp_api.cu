@@ -823,7 +823,6 @@ dedisp_status dedisp_stream_push_host(dedisp_stream* s, const void* host_chunk_i
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     dedisp_plan* p = s->plan;
     const size_t es = in_size(s->dtype);
-    const size_t nin = static_cast<size_t>(s->nbeams) * p->nchans * s->chunk * es;
     const size_t nout = static_cast<size_t>(s->nbeams) * p->ndm * s->chunk * 4;
     if (s->chunk % 4 != 0)
         return DEDISP_ESHAPE;

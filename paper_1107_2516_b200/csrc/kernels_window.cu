@@ -109,13 +109,6 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
                  "l"(src), "r"(bytes), "r"(bar)
                  : "memory");
 }
-// in place (tied operand): with a separate destination ptxas adds into a fresh register pair and
-// copies it back when registers are short (4 IMAD.MOV per channel at 160 registers)
-__device__ __forceinline__ void add2(u64& a, u64 b)
-{
-    asm volatile("add.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(b));
-}
-
 #include "window_rows.inc"
 
 // ------------------------------------------------------------------------------------------------
@@ -297,12 +290,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         if (sm >> 7)
             shift_rows<T, D>(acc, sm >> 7, lane_pinned);
     };
-    auto adds = [&](u64(&w)[T + 1], unsigned m) {
-#pragma unroll
-        for (int k = 0; k < T; ++k)
-            add2(acc[0][k], w[k]);
-        rows7(acc, w, m);
-    };
+    auto adds = [&](u64(&w)[T + 1], unsigned m) { rows7(acc, w, m); };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
     // accumulator registers between copies otherwise).  The bookkeeping that runs once per channel
     // is kept to the window address and the rotation of the stage's four metadata words: every
