@@ -124,13 +124,25 @@ __global__ void __launch_bounds__(kDetThreads) detect_emit_kernel(const T* __res
     const int64_t n4 = n / 4;
     for (int d = blockIdx.x; d < ndm; d += gridDim.x) {
         const T* row = base + static_cast<int64_t>(d) * stride;
-        for (int64_t q = threadIdx.x; q < n4; q += kDetThreads) {
-            const int4 raw = *reinterpret_cast<const int4*>(row + 4 * q);
-            const T* v = reinterpret_cast<const T*>(&raw);
+        // four 16-byte loads in flight per thread before any test
+        for (int64_t q0 = threadIdx.x; q0 < n4; q0 += 4 * kDetThreads) {
+            int4 raw[4];
 #pragma unroll
-            for (int k = 0; k < 4; ++k)
-                if (to_f64(v[k]) > thr)
-                    emit(4 * q + k, d, v[k]);
+            for (int u = 0; u < 4; ++u) {
+                const int64_t q = q0 + u * kDetThreads;
+                raw[u] = q < n4 ? *reinterpret_cast<const int4*>(row + 4 * q) : make_int4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int64_t q = q0 + u * kDetThreads;
+                if (q >= n4)
+                    break;
+                const T* v = reinterpret_cast<const T*>(&raw[u]);
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (to_f64(v[k]) > thr)
+                        emit(4 * q + k, d, v[k]);
+            }
         }
         for (int64_t t = 4 * n4 + threadIdx.x; t < n; t += kDetThreads)
             if (to_f64(row[t]) > thr)

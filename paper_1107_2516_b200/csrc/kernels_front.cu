@@ -48,27 +48,40 @@ __global__ void __launch_bounds__(256) power_corner_turn_kernel(const float2* __
 
 // Binning, stage (i) of the subband scheme ("Binning averages N_b consecutive samples"):
 // out[c][j] = (in[c][j*nb] + ... + in[c][j*nb + nb-1]) / nb, the sum left to right, every operation
-// rounded on its own.  One thread per output; a warp reads 32*nb consecutive floats.  HBM-bound.
+// rounded on its own.  Four outputs per thread, 256 apart; a warp reads 32*nb consecutive floats per output.  HBM-bound.
 __global__ void __launch_bounds__(256) bin_kernel(const float* __restrict__ in, float* __restrict__ out, int64_t nout,
                                                   int64_t in_stride, int64_t out_stride, int nb, int vec)
 {
-    const int64_t j = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
-    if (j >= nout)
-        return;
-    const float* p = in + static_cast<int64_t>(blockIdx.y) * in_stride + j * nb;
-    float acc;
-    if (nb == 2 && vec) {  // the paper's bin factors (Table 1: 1, 2, 4) with one vector load, same order of adds
-        const float2 v = *reinterpret_cast<const float2*>(p);
-        acc = __fadd_rn(v.x, v.y);
-    } else if (nb == 4 && vec) {
-        const float4 v = *reinterpret_cast<const float4*>(p);
-        acc = __fadd_rn(__fadd_rn(__fadd_rn(v.x, v.y), v.z), v.w);
-    } else {
-        acc = p[0];
-        for (int i = 1; i < nb; ++i)
-            acc = __fadd_rn(acc, p[i]);
+    // four outputs per thread, 256 apart (coalesced), so that enough loads are in flight
+    const int64_t j0 = static_cast<int64_t>(blockIdx.x) * 1024 + threadIdx.x;
+    const float* row = in + static_cast<int64_t>(blockIdx.y) * in_stride;
+    float acc[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int64_t j = j0 + 256 * k;
+        acc[k] = 0.0f;
+        if (j >= nout)
+            continue;
+        const float* p = row + j * nb;
+        if (nb == 2 && vec) {  // the paper's bin factors (Table 1: 1, 2, 4) with one vector load, same order of adds
+            const float2 v = *reinterpret_cast<const float2*>(p);
+            acc[k] = __fadd_rn(v.x, v.y);
+        } else if (nb == 4 && vec) {
+            const float4 v = *reinterpret_cast<const float4*>(p);
+            acc[k] = __fadd_rn(__fadd_rn(__fadd_rn(v.x, v.y), v.z), v.w);
+        } else {
+            float a = p[0];
+            for (int i = 1; i < nb; ++i)
+                a = __fadd_rn(a, p[i]);
+            acc[k] = a;
+        }
     }
-    out[static_cast<int64_t>(blockIdx.y) * out_stride + j] = __fdiv_rn(acc, static_cast<float>(nb));
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int64_t j = j0 + 256 * k;
+        if (j < nout)
+            out[static_cast<int64_t>(blockIdx.y) * out_stride + j] = __fdiv_rn(acc[k], static_cast<float>(nb));
+    }
 }
 
 }  // namespace
@@ -83,7 +96,7 @@ int launch_bin(const void* in, void* out, int64_t nrows, int64_t nout, int64_t i
     const int vec = (nb == 2 || nb == 4) && in_stride % nb == 0 && (reinterpret_cast<uintptr_t>(in) % (4 * nb)) == 0;
     for (int64_t r0 = 0; r0 < nrows; r0 += 65535) {  // grid.y limit
         const int64_t nr = nrows - r0 < 65535 ? nrows - r0 : 65535;
-        dim3 grid(static_cast<unsigned>((nout + 255) / 256), static_cast<unsigned>(nr));
+        dim3 grid(static_cast<unsigned>((nout + 1023) / 1024), static_cast<unsigned>(nr));
         bin_kernel<<<grid, 256, 0, st>>>(static_cast<const float*>(in) + r0 * in_stride,
                                          static_cast<float*>(out) + r0 * out_stride, nout, in_stride, out_stride, nb, vec);
     }
