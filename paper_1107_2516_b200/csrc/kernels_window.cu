@@ -209,30 +209,31 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         // ---- producer warp group: gives its registers to the consumers; one thread stages kWinCh
         // channels per barrier (padding channels and the extra last stage get zeros)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
-        if (warp == NCW) {
+        {
+            // the four warps of the group take the stages in turn (stage s belongs to warp s % 4), so
+            // the staging work is spread over the four schedulers instead of loading the one that also
+            // runs consumer warps 0, 4, 8
+            const int pw = warp - NCW;
             const int32_t* meta = a.meta + (static_cast<int64_t>(ty) * a.nchans + c_begin) * kWinMetaWords;
             const int32_t* hdr = a.hdr + (static_cast<int64_t>(ty) * stage_total + stage0) * kWinHdrWords;
             const float2* prow = static_cast<const float2*>(a.pairs) +
                                  (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
             const int64_t pair_stride = a.pair_stride;
             const int zlen = ((NT - 1) * a.H + W + 2 + 1) & ~1;  // pairs a padding channel must provide
-            int pb = 0, pl = 0;  // lane L: (base, len) of channel 32*q + L
-            int ring = 0, lap = 0;
-            for (int s = 0; s < nstage; ++s) {
-                if ((s & 7) == 0) {  // 8 stages = 32 channels per metadata fetch
-                    const int k = s * kWinCh + lane;
-                    pb = 0;
-                    pl = -1;
-                    if (k < nch) {
-                        pb = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords);
-                        pl = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords + 1);
-                    }
+            for (int s = pw; s < nstage; s += 4) {
+                const int ring = s % nst, lap = s / nst;
+                // lanes 0 .. kWinCh-1: (base, len) of this stage's channels
+                const int k = s * kWinCh + lane;
+                int pb = 0, pl = -1;
+                if (lane < kWinCh && k < nch) {
+                    pb = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords);
+                    pl = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords + 1);
                 }
                 int base[kWinCh], len[kWinCh];
 #pragma unroll
                 for (int ch = 0; ch < kWinCh; ++ch) {
-                    base[ch] = __shfl_sync(0xffffffffu, pb, ((s & 7) * kWinCh + ch) & 31);
-                    len[ch] = __shfl_sync(0xffffffffu, pl, ((s & 7) * kWinCh + ch) & 31);
+                    base[ch] = __shfl_sync(0xffffffffu, pb, ch);
+                    len[ch] = __shfl_sync(0xffffffffu, pl, ch);
                 }
                 if (lane == 0) {
                     if (lap > 0)
@@ -256,10 +257,6 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
                     }
                 }
                 __syncwarp();
-                if (++ring == nst) {
-                    ring = 0;
-                    ++lap;
-                }
             }
         }
         return;
