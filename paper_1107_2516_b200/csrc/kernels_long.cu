@@ -11,7 +11,7 @@
 // and that union is only well used when the tile is long compared with the spread of the rows'
 // delays.  Hence the shape: R = 16 rows (one consumer warp each) x L = 32*TT = 2048 samples, the
 // accumulators of a row in the registers of its warp (lane owns samples lane + 32 i: conflict-free for
-// any delay), and one producer warp that computes the union per channel and stages it with a 1-D TMA
+// any delay), and four producer warps (one per scheduler, channels in turn) that compute the union per channel and stages it with a 1-D TMA
 // bulk copy (cp.async.bulk + mbarrier) into a ring of shared-memory slots.  On cfg 4's stage 1 a
 // staged word then serves 16*2048/(2048 + 16*~70) ~ 10 adds instead of 1.7 in the 32 x 256 tile of
 // direct_kernel (which drew 8.4 TB/s from L2 and was bound by that).
@@ -63,11 +63,13 @@ __device__ __forceinline__ void tma_g2s(unsigned dst, const void* src, unsigned 
                  : "memory");
 }
 
+constexpr int kLongProducers = 4;  // staging warps, one per scheduler: channel c belongs to warp c % 4
+
 // shared memory: full[nslot], empty[nslot] (mbarriers) | offs[nslot][R] | slots[nslot][cap] InT
 __host__ __device__ inline int long_hdr_bytes(int nslot, int R) { return (16 * nslot + 4 * R * nslot + 127) & ~127; }
 
 template <typename InT, int R, int TT>
-__global__ void __launch_bounds__((R + 1) * 32, 1) long_kernel(const Problem p, const int cap, const int nslot, const int nrt)
+__global__ void __launch_bounds__((R + kLongProducers) * 32, 1) long_kernel(const Problem p, const int cap, const int nslot, const int nrt)
 {
     using AccT = typename AccOfL<InT>::type;
     constexpr int L = 32 * TT;
@@ -105,11 +107,14 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) long_kernel(const Problem p, 
     }
     __syncthreads();
 
-    if (warp == R) {
-        // ---- producer: per channel the union of the active rows' sample ranges, one bulk copy
+    if (warp >= R) {
+        // ---- producers: per channel the union of the active rows' sample ranges, one bulk copy.  The
+        // staging work (16 shuffles and a min/max per channel) is spread over four warps, one per
+        // scheduler: a single producer warp made its scheduler (which also runs four consumer warps)
+        // the slowest and gated the ring.
+        const int pw = warp - R;
         const InT* in = static_cast<const InT*>(p.in) + b0 * p.in_b0_stride + b1 * p.in_b1_stride;
         const int32_t* sh = p.shift + b1 * p.shift_b1_stride;
-        int ring = 0, lap = 0;
         for (int c0 = 0; c0 < p.nchans; c0 += 32) {
             int sv[R];  // lane l: shift(d0 + j, c0 + l)
 #pragma unroll
@@ -118,7 +123,9 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) long_kernel(const Problem p, 
                             ? __ldg(sh + static_cast<int64_t>(d0 + j) * p.shift_dm_stride + c0 + lane)
                             : 0;
             const int nc = p.nchans - c0 < 32 ? p.nchans - c0 : 32;
-            for (int i = 0; i < nc; ++i) {
+            for (int i = pw; i < nc; i += kLongProducers) {
+                const int c = c0 + i;
+                const int ring = c % nslot, lap = c / nslot;
                 int mn = INT_MAX, mx = 0, mine = 0;
 #pragma unroll
                 for (int j = 0; j < R; ++j) {
@@ -145,15 +152,11 @@ __global__ void __launch_bounds__((R + 1) * 32, 1) long_kernel(const Problem p, 
                     if (nv > 0) {
                         bar_expect_tx(fb, static_cast<unsigned>(nv) * 16u);
                         tma_g2s(smem_addr(smem + hdr) + ring * slot_bytes,
-                                in + static_cast<int64_t>(c0 + i) * p.in_chan_stride + g,
+                                in + static_cast<int64_t>(c) * p.in_chan_stride + g,
                                 static_cast<unsigned>(nv) * 16u, fb);
                     } else {
                         bar_arrive(fb);
                     }
-                }
-                if (++ring == nslot) {
-                    ring = 0;
-                    ++lap;
                 }
             }
         }
@@ -225,7 +228,7 @@ int launch_long_t(const Problem& p, int spread, cudaStream_t st)
     if (e != cudaSuccess)
         return static_cast<int>(e);
     dim3 grid(static_cast<unsigned>(ntt * nrt), p.nb1, p.nb0);
-    long_kernel<InT, R, TT><<<grid, (R + 1) * 32, smem, st>>>(p, static_cast<int>(cap), nslot, nrt);
+    long_kernel<InT, R, TT><<<grid, (R + kLongProducers) * 32, smem, st>>>(p, static_cast<int>(cap), nslot, nrt);
     return static_cast<int>(cudaGetLastError());
 }
 
