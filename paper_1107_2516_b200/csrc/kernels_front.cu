@@ -25,19 +25,19 @@ __global__ void __launch_bounds__(256) power_corner_turn_kernel(const float2* __
     const int tx = threadIdx.x & 63, ty = threadIdx.x >> 6;  // 64 x 4 threads
     const int64_t t0 = static_cast<int64_t>(blockIdx.x) * kTile;
     const int c0 = blockIdx.y * kTile;
-#pragma unroll 4
-    for (int k = ty; k < kTile; k += 4) {
-        const int64_t t = t0 + k;
+    // all 16 loads of a thread in flight before the first square
+    float2 v[kTile / 4];
+#pragma unroll
+    for (int q = 0; q < kTile / 4; ++q) {
+        const int64_t t = t0 + ty + 4 * q;
         const int c = c0 + tx;
-        float p = 0.0f;
-        if (t < nsamp && c < nchans) {
-            const float2 v = volt[t * volt_stride + c];
-            p = __fadd_rn(__fmul_rn(v.x, v.x), __fmul_rn(v.y, v.y));
-        }
-        tile[k][tx] = p;
+        v[q] = t < nsamp && c < nchans ? volt[t * volt_stride + c] : make_float2(0.0f, 0.0f);
     }
+#pragma unroll
+    for (int q = 0; q < kTile / 4; ++q)
+        tile[ty + 4 * q][tx] = __fadd_rn(__fmul_rn(v[q].x, v[q].x), __fmul_rn(v[q].y, v[q].y));
     __syncthreads();
-#pragma unroll 4
+#pragma unroll
     for (int k = ty; k < kTile; k += 4) {
         const int c = c0 + k;
         const int64_t t = t0 + tx;
