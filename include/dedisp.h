@@ -18,10 +18,19 @@
  *     buffers are owned by the library and released by the matching *_destroy.
  *   - Data layout: input is channel-major and time-contiguous, channel 0 is the
  *     highest frequency f_top, channel c is at f_top - c*df.  Batches ("beams") are outermost.
- *   - dedisp_execute / dedisp_stream_push enqueue work on the given cudaStream_t and return
- *     without synchronising.  Argument errors are reported synchronously; a CUDA launch error
- *     is reported as DEDISP_ECUDA by the call that saw it.
- *   - No exceptions cross this boundary, nothing calls exit(), there is no global state.
+ *   - dedisp_execute / dedisp_stream_push / dedisp_plan_detect enqueue work on the given
+ *     cudaStream_t and return without synchronising, allocating or freeing: device tables and
+ *     scratch are set up beforehand by dedisp_plan_reserve (blocking).  Argument errors are
+ *     reported synchronously; a CUDA launch error is reported as DEDISP_ECUDA by the call that
+ *     saw it.  The *_host entries and *_create / *_reserve / *_destroy may allocate and block.
+ *   - A plan's tables are immutable after creation.  Its scratch (pair buffer, subband
+ *     intermediate, detection workspace) and its bookkeeping (last_launches, timing events) are
+ *     per plan: ONE execute / push / detect per plan may be in flight at a time, for both kinds
+ *     of plan, and calls on one plan must not be made from several threads at once.  Use one
+ *     plan per CUDA stream for concurrent work.  A plan lives on the device that was current at
+ *     its first dedisp_plan_reserve.
+ *   - No exceptions cross this boundary, nothing calls exit(), there is no global state and the
+ *     library reads no environment variables.
  *   - There is no CPU fallback: without a CUDA device every execute/push returns DEDISP_ECUDA.
  *     Plan creation and the table getters are host-only and work without a device.
  */
@@ -116,8 +125,9 @@ DEDISP_API int dedisp_plan_nfine(const dedisp_plan *plan);
 DEDISP_API dedisp_status dedisp_plan_get_shifts(const dedisp_plan *plan, int32_t *host_out);
 
 /* Subband plans: s1 [ncoarse][nchans], s2 [ndm][nsub], nominal_dm [ncoarse],
- * maxshift2 [ncoarse] (overlap stage 1 keeps for stage 2); all HOST; any may be
- * NULL.  DEDISP_ESTATE for brute-force plans. */
+ * maxshift2 [ncoarse] (overlap stage 1 keeps for stage 2; one argument more than
+ * SURVEY.md section 8b's sketch of this call); all HOST; any may be NULL.  DEDISP_ESTATE for
+ * brute-force plans. */
 DEDISP_API dedisp_status dedisp_plan_get_subband_shifts(const dedisp_plan *plan, int32_t *s1, int32_t *s2,
                                              double *nominal_dm, int32_t *maxshift2);
 
@@ -128,13 +138,34 @@ DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel
 /* Which kernel AUTO resolves to for this plan and dtype (a dedisp_kernel value), -1 on error. */
 DEDISP_API int dedisp_plan_resolved_kernel(const dedisp_plan *plan, dedisp_dtype dtype);
 
-/* Geometry the register-window kernel would use for this plan, 8 int64 to HOST memory:
- * [0] 1 if the plan's table fits the kernel (else the rest is 0), [1] H: a warp emits the sample
- * pairs (t, t+H) of H consecutive t per DM row, [2] largest number of row shifts in a channel band
- * (slots lost per warp tile), [3] longest staged channel segment in pairs, [4] DM tiles,
- * [5] slots per row and warp, [6] DM rows per block, [7] channel bands (= kernel launches).
+/* Geometry the register-window kernel would use for this plan, 12 int64 to HOST memory:
+ * [0] 1 if the plan's table fits the kernel (else the rest is 0), [1] Hb: output samples per
+ * block and DM row (blocks are Hb apart in time), [2] kmax: largest number of row shifts in a
+ * channel band = samples a block loses, Hb = 2*NT*W - kmax, [3] longest staged channel segment
+ * in pairs, [4] DM tiles, [5] W: slots per row and warp segment, [6] DM rows per block,
+ * [7] channel bands (= kernel launches), [8] T, [9] G, [10] NT, [11] D (below).
  * Brute-force plans only carry one. */
 DEDISP_API dedisp_status dedisp_plan_window_info(const dedisp_plan *plan, int64_t *info);
+
+/* Tuning knob: thread / block shape of the register-window kernel.  A thread owns D DM rows x T
+ * sample pairs, a block G row groups x NT warps along time.  Only the instantiated shapes are
+ * accepted (DEDISP_EINVAL otherwise): (T,G,NT,D) = (15,6,2,4) [default], (15,4,3,4), (21,4,1,4),
+ * (21,8,1,4), (17,4,1,5), (15,4,1,6), (11,8,1,8).  Brute-force plans, before the first
+ * dedisp_plan_reserve (DEDISP_ESTATE otherwise, or when the table does not fit the shape: the
+ * plan then keeps the shape it had).  Results do not depend on it beyond fp32 summation order. */
+DEDISP_API dedisp_status dedisp_plan_set_window_geometry(dedisp_plan *plan, int T, int G, int NT, int D);
+
+/*
+ * dedisp_plan_reserve -- copy the plan's tables to the current device (first call) and size its
+ * scratch for executes / pushes / detects of up to nsamp_out output samples and nbeams beams of
+ * dtype: the pair buffer of the register-window kernel (2 x 4 bytes per input sample), the subband
+ * intermediate (dedisp_plan_scratch_bytes), the detection workspace.  Blocking (cudaMalloc,
+ * cudaMemcpy); may be called again with a larger shape while nothing is in flight.  Must precede
+ * dedisp_execute / dedisp_plan_detect; dedisp_stream_create and the *_host entries call it
+ * themselves.  Errors: DEDISP_EINVAL, DEDISP_ENOMEM, DEDISP_ECUDA, DEDISP_ESTATE (the plan lives
+ * on another device).
+ */
+DEDISP_API dedisp_status dedisp_plan_reserve(dedisp_plan *plan, dedisp_dtype dtype, int64_t nsamp_out, int nbeams);
 
 /* Bytes of device scratch a subband execute of nsamp_out samples and nbeams beams needs
  * (the stage-1 intermediate, fp32 or int32); 0 for brute-force plans; -1 on error. */
@@ -153,10 +184,11 @@ DEDISP_API int64_t dedisp_plan_scratch_bytes(const dedisp_plan *plan, int64_t ns
  *
  * Brute-force plans: the register-window kernel (a pair-forming pre-pass into plan-owned scratch,
  * then one launch per channel band) or one long-tile / direct launch.  Subband plans: stage 1
- * into the plan's scratch (grown on demand, so one execute per plan may be in flight), then
- * stage 2; stage 1 forms of every (group, subband) series only the samples stage 2 reads.  Input elements beyond
- * nsamp_out + max_delay in a row are never read; output elements beyond nsamp_out in a row are
- * never written.  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ENOMEM, DEDISP_ECUDA.
+ * into the plan's scratch, then stage 2; stage 1 forms of every (group, subband) series only the
+ * samples stage 2 reads.  Input elements beyond nsamp_out + max_delay in a row are never read;
+ * output elements beyond nsamp_out in a row are never written.  Asynchronous: no allocation, no
+ * synchronisation.  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ECUDA, DEDISP_ESTATE (no
+ * dedisp_plan_reserve covering dtype / nsamp_out / nbeams, or another device is current).
  */
 DEDISP_API dedisp_status dedisp_execute(dedisp_plan *plan, const void *in, void *out, dedisp_dtype dtype,
                              int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
@@ -235,8 +267,9 @@ DEDISP_API dedisp_status dedisp_plan_last_stage_ms(dedisp_plan *plan, float *ms)
  *              valid, in no particular order
  *   results    DEVICE, [nbeams]; count is the number of outputs above the threshold (it may exceed
  *              capacity: the surplus is counted, not stored)
- * Asynchronous on cuda_stream; the plan owns a small workspace (one detect per plan in flight).
- * Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ENOMEM, DEDISP_ECUDA.
+ * Asynchronous on cuda_stream; the plan owns a small workspace sized by dedisp_plan_reserve (one
+ * detect per plan in flight).  Errors: DEDISP_EINVAL, DEDISP_ESHAPE, DEDISP_ECUDA, DEDISP_ESTATE
+ * (no dedisp_plan_reserve for this many beams).
  */
 typedef struct { int64_t t; int32_t dm; float value; } dedisp_event;            /* 16 bytes */
 typedef struct { double mean, sigma, threshold; int64_t count; } dedisp_detect_result;

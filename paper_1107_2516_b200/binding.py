@@ -30,6 +30,8 @@ _SIGS = {
     "dedisp_plan_set_kernel": (_int, [_vp, _int]),
     "dedisp_plan_resolved_kernel": (_int, [_vp, _int]),
     "dedisp_plan_window_info": (_int, [_vp, _vp]),
+    "dedisp_plan_set_window_geometry": (_int, [_vp, _int, _int, _int, _int]),
+    "dedisp_plan_reserve": (_int, [_vp, _int, _i64, _int]),
     "dedisp_plan_scratch_bytes": (_i64, [_vp, _i64, _int]),
     "dedisp_execute": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _vp]),
     "dedisp_execute_host": (_int, [_vp, _vp, _vp, _int, _i64, _int, _vp]),
@@ -107,6 +109,20 @@ class Plan:
                                         int(dm.size), int(nsub), int(nfine)), "dedisp_plan_create")
         self._h = h
         self.nchans, self.ndm, self.nsub, self.nfine = int(nchans), int(dm.size), int(nsub), int(nfine)
+        self._reserved = {}
+
+    def reserve(self, dtype, nsamp_out, nbeams=1):
+        """dedisp_plan_reserve: tables onto the current device, scratch for this shape (blocking)."""
+        _check(lib().dedisp_plan_reserve(self._h, int(dtype), int(nsamp_out), int(nbeams)), "dedisp_plan_reserve")
+        n, b = self._reserved.get(int(dtype), (0, 0))
+        self._reserved[int(dtype)] = (max(n, int(nsamp_out)), max(b, int(nbeams)))
+
+    def _ensure_reserved(self, dtype, nsamp_out, nbeams):
+        # execute / detect never allocate (include/dedisp.h): the binding reserves the first time a
+        # shape is seen, which keeps `plan.execute(x, n)` a one-liner
+        n, b = self._reserved.get(int(dtype), (-1, 0))
+        if nsamp_out > n or nbeams > b:
+            self.reserve(dtype, max(n, int(nsamp_out)), max(b, int(nbeams)))
 
     def close(self):
         if getattr(self, "_h", None):
@@ -141,15 +157,20 @@ class Plan:
 
     def set_kernel(self, kernel):
         _check(lib().dedisp_plan_set_kernel(self._h, int(kernel)), "dedisp_plan_set_kernel")
+        self._reserved = {}          # the scratch a shape needs depends on the kernel
+
+    def set_window_geometry(self, T, G, NT, D):
+        _check(lib().dedisp_plan_set_window_geometry(self._h, int(T), int(G), int(NT), int(D)),
+               "dedisp_plan_set_window_geometry")
 
     def resolved_kernel(self, dtype=F32):
         return int(lib().dedisp_plan_resolved_kernel(self._h, int(dtype)))
 
     def window_info(self):
         """dedisp_plan_window_info as a dict (geometry of the register-window kernel)."""
-        a = np.zeros(8, dtype=np.int64)
+        a = np.zeros(12, dtype=np.int64)
         _check(lib().dedisp_plan_window_info(self._h, a.ctypes.data), "dedisp_plan_window_info")
-        keys = ("ok", "H", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "nband")
+        keys = ("ok", "Hb", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "nband", "T", "G", "NT", "D")
         return dict(zip(keys, (int(v) for v in a)))
 
     def scratch_bytes(self, nsamp_out, nbeams=1):
@@ -197,6 +218,7 @@ class Plan:
             if out3.dtype != odt or out3.stride(2) != 1 or out3.shape[1] != self.ndm or \
                     (nb > 1 and out3.stride(0) != self.ndm * out3.stride(1)):
                 raise DedispError(ESHAPE, "dedisp_execute")
+        self._ensure_reserved(dt, int(nsamp_out), int(nb))
         _check(lib().dedisp_execute(self._h, x3.data_ptr(), out3.data_ptr(), dt, int(nsamp_out),
                                     int(x3.stride(1)), int(out3.stride(1)), int(nb), _stream_ptr(stream)),
                "dedisp_execute")
@@ -211,6 +233,7 @@ class Plan:
         assert o.is_cuda and o.stride(2) == 1 and o.shape[1] == self.ndm and o.stride(0) == o.stride(1) * self.ndm
         dt = F32 if o.dtype == torch.float32 else U8
         nb = o.shape[0]
+        self._ensure_reserved(dt, 0, int(nb))
         ev = torch.zeros((nb, capacity, 4), dtype=torch.int32, device=o.device)     # 16-byte records
         res = torch.zeros((nb, 4), dtype=torch.float64, device=o.device)            # 32-byte records
         _check(lib().dedisp_plan_detect(self._h, o.data_ptr(), dt, int(o.shape[2]), int(o.stride(1)), int(nb),

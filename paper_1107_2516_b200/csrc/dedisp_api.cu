@@ -80,7 +80,7 @@ struct dedisp_plan {
     int spread_s1[3] = {0, 0, 0}, spread_s2[3] = {0, 0, 0};
     // device side (uploaded by the first execute)
     bool uploaded = false;
-    int device = -1;
+    int device = -1, nsm = 148;
     int32_t *d_shift = nullptr, *d_s1 = nullptr, *d_s2 = nullptr, *d_maxshift2 = nullptr, *d_maxshift2_ks = nullptr;
     DevBuf scratch;            // subband intermediate
     DevBuf host_in, host_out;  // staging for dedisp_execute_host
@@ -115,17 +115,37 @@ struct dedisp_stream {
     DevBuf host_in, host_out;
 };
 
+extern "C" int64_t dedisp_plan_scratch_bytes(const dedisp_plan* p, int64_t nsamp_out, int nbeams);
+
 namespace {
 
 size_t in_size(dedisp_dtype t) { return t == DEDISP_F32 ? 4 : 1; }
 
+void free_tables(dedisp_plan* p)
+{
+    int32_t** tabs[] = {&p->d_shift, &p->d_s1, &p->d_s2, &p->d_maxshift2, &p->d_maxshift2_ks,
+                        &p->d_win_meta, &p->d_win_kfinal, &p->d_win_theta, &p->d_win_hdr};
+    for (int32_t** t : tabs) {
+        if (*t)
+            cudaFree(*t);
+        *t = nullptr;
+    }
+    if (p->d_win_zeros)
+        cudaFree(p->d_win_zeros);
+    p->d_win_zeros = nullptr;
+    p->uploaded = false;
+}
+
+// copies the plan's tables to the current device (blocking; called by dedisp_plan_reserve only)
 dedisp_status upload(dedisp_plan* p)
 {
-    if (p->uploaded)
-        return DEDISP_OK;
     int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess)
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
         return DEDISP_ECUDA;
+    }
+    if (p->uploaded)
+        return dev == p->device ? DEDISP_OK : DEDISP_ESTATE;  // a plan lives on one device
     auto up = [](int32_t** d, const std::vector<int32_t>& h) -> cudaError_t {
         if (h.empty())
             return cudaSuccess;
@@ -163,16 +183,21 @@ dedisp_status upload(dedisp_plan* p)
     }
     if (e != cudaSuccess) {
         cudaGetLastError();
+        free_tables(p);  // nothing stays behind for a retry to leak
         return e == cudaErrorMemoryAllocation ? DEDISP_ENOMEM : DEDISP_ECUDA;
     }
     p->device = dev;
+    cudaDeviceGetAttribute(&p->nsm, cudaDevAttrMultiProcessorCount, dev);
     p->uploaded = true;
     return DEDISP_OK;
 }
 
-bool use_window(const dedisp_plan* p, dedisp_dtype dtype)
+bool use_window(const dedisp_plan* p, dedisp_dtype dtype, int64_t nsamp_out)
 {
     if (p->nsub != 0 || !p->win.ok || !p->win_fits)
+        return false;
+    // the kernel keeps output times in 32 bits
+    if (nsamp_out > 0 && window_pair_stride(p->win, nsamp_out) >= (1LL << 30))
         return false;
     // uint8 sums are carried in fp32, exact while nchans * 255 < 2^24
     if (dtype == DEDISP_U8 && static_cast<int64_t>(p->nchans) * 255 >= (1 << 24))
@@ -187,11 +212,8 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     WindowArgs a;
     std::memset(&a, 0, sizeof(a));
     a.pair_stride = window_pair_stride(plan->win, nsamp_out);
-    const size_t need = static_cast<size_t>(nbeams) * plan->nchans * a.pair_stride * 8;
-    if (plan->pairs.ensure(need) != cudaSuccess) {
-        cudaGetLastError();
-        return DEDISP_ENOMEM;
-    }
+    if (static_cast<size_t>(nbeams) * plan->nchans * a.pair_stride * 8 > plan->pairs.bytes)
+        return DEDISP_ESTATE;  // dedisp_plan_reserve was not called for this shape
     a.in = in;
     a.out = out;
     a.pairs = plan->pairs.p;
@@ -216,7 +238,8 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.nchans = plan->nchans;
     a.ndm = plan->ndm;
     a.nbeams = nbeams;
-    a.H = plan->win.H;
+    a.Hb = plan->win.Hb;
+    a.kmax = plan->win.kmax;
     a.lmax = plan->win.lmax;
     a.ntile_dm = plan->win.ntile_dm;
     a.ntile_t = static_cast<int>(window_ntile_t(plan->win, nsamp_out));
@@ -224,10 +247,8 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
         // DM tiles per block-order group: a wave of `inflight` blocks = g DM tiles x inflight/g time
         // tiles reads about g * cols_per_tile + (inflight / g) * tile_cols columns of the pair buffer;
         // the g that minimises it
-        int nsm = 148;
-        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, plan->device);
-        const double inflight = nsm * (plan->win.geom.G * plan->win.geom.NT == 4 ? 2.0 : 1.0);
-        const double tile_cols = 2.0 * plan->win.geom.NT * plan->win.H;
+        const double inflight = plan->nsm * (plan->win.geom.G * plan->win.geom.NT == 4 ? 2.0 : 1.0);
+        const double tile_cols = plan->win.Hb;
         double mean_last = 0.0;  // mean over channels of the largest delay
         const int32_t* last = plan->shift.data() + static_cast<size_t>(plan->ndm - 1) * plan->nchans;
         for (int c = 0; c < plan->nchans; ++c)
@@ -236,8 +257,6 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
         const double cols_per_tile = mean_last / plan->win.ntile_dm + 1.0;
         int g = static_cast<int>(std::sqrt(inflight * tile_cols / cols_per_tile) + 0.5);
         g = g < 1 ? 1 : g > plan->win.ntile_dm ? plan->win.ntile_dm : g;
-        if (const char* e = std::getenv("DEDISP_WINDOW_DMGROUP"))  // development override
-            g = std::atoi(e) > 0 ? std::atoi(e) : g;
         a.dm_group = g > plan->win.ntile_dm ? plan->win.ntile_dm : g;
     }
     return launch_window(a, in_t, stream, &plan->last_launches) == 0 ? DEDISP_OK : DEDISP_ECUDA;
@@ -279,17 +298,20 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
         (reinterpret_cast<uintptr_t>(out) & 15) != 0)
         return DEDISP_ESHAPE;
     plan->last_launches = 0;
-    dedisp_status st = upload(plan);
-    if (st != DEDISP_OK)
-        return st;
+    {
+        // never allocates, never blocks: tables and scratch come from dedisp_plan_reserve
+        int dev = -1;
+        if (!plan->uploaded || cudaGetDevice(&dev) != cudaSuccess || dev != plan->device)
+            return DEDISP_ESTATE;
+    }
     const Elem in_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::U8;
 
     Problem pr;
     std::memset(&pr, 0, sizeof(pr));
     pr.nb0 = nbeams;
-    pr.in_len = in_stride;
+    pr.in_len = nsamp_out + plan->max_delay;  // the extent seen from `in`: nothing beyond it is read
     int rc = 0;
-    if (use_window(plan, dtype))
+    if (use_window(plan, dtype, nsamp_out))
         return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream);
     struct Timer {  // the direct / subband kernels are timed as a whole
         dedisp_plan* p;
@@ -327,11 +349,8 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     // two-stage subband: stage 1 into scratch, stage 2 from scratch
     const int ncoarse = plan->ndm / plan->nfine, cps = plan->nchans / plan->nsub;
     const int64_t n1 = round_up(nsamp_out + plan->maxshift2_max, 16);
-    const size_t need = static_cast<size_t>(nbeams) * ncoarse * plan->nsub * n1 * 4;
-    if (plan->scratch.ensure(need) != cudaSuccess) {
-        cudaGetLastError();
-        return DEDISP_ENOMEM;
-    }
+    if (static_cast<size_t>(nbeams) * ncoarse * plan->nsub * n1 * 4 > plan->scratch.bytes)
+        return DEDISP_ESTATE;  // dedisp_plan_reserve was not called for this shape
     // stage 1: b1 = subband s, rows = coarse groups k, channels = the cps channels of s
     pr.in = in;
     pr.out = plan->scratch.p;
@@ -382,6 +401,30 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     p2.nb1 = ncoarse;
     rc = run_problem(plan, p2, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, plan->spread_s2, stream);
     return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+// tables onto the current device, scratch for executes of up to nsamp_out x nbeams (blocking)
+dedisp_status reserve(dedisp_plan* plan, dedisp_dtype dtype, int64_t nsamp_out, int nbeams)
+{
+    if (!plan || nbeams <= 0 || nsamp_out < 0 || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    dedisp_status st = upload(plan);
+    if (st != DEDISP_OK)
+        return st;
+    size_t pairs = 0, scratch = 0;
+    if (plan->nsub == 0) {
+        if (use_window(plan, dtype, nsamp_out) && nsamp_out > 0)
+            pairs = static_cast<size_t>(nbeams) * plan->nchans * window_pair_stride(plan->win, nsamp_out) * 8;
+    } else {
+        scratch = static_cast<size_t>(dedisp_plan_scratch_bytes(plan, nsamp_out, nbeams));
+    }
+    const size_t det = static_cast<size_t>(nbeams) * detect_blocks(plan->ndm) * 2 * sizeof(double);
+    if (plan->pairs.ensure(pairs) != cudaSuccess || plan->scratch.ensure(scratch) != cudaSuccess ||
+        plan->det_partial.ensure(det) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    return DEDISP_OK;
 }
 
 bool ensure_copy_streams(dedisp_plan* plan)
@@ -484,18 +527,7 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
         return DEDISP_OK;
     if (p->nstreams != 0)
         return DEDISP_ESTATE;
-    if (p->uploaded) {
-        cudaFree(p->d_shift);
-        cudaFree(p->d_s1);
-        cudaFree(p->d_s2);
-        cudaFree(p->d_maxshift2);
-        cudaFree(p->d_maxshift2_ks);
-        cudaFree(p->d_win_meta);
-        cudaFree(p->d_win_kfinal);
-        cudaFree(p->d_win_theta);
-        cudaFree(p->d_win_hdr);
-        cudaFree(p->d_win_zeros);
-    }
+    free_tables(p);
     if (p->ev[0])
         cudaEventDestroy(p->ev[0]);
     if (p->ev[1])
@@ -604,11 +636,32 @@ dedisp_status dedisp_plan_set_kernel(dedisp_plan* p, dedisp_kernel k)
     return DEDISP_OK;
 }
 
+dedisp_status dedisp_plan_set_window_geometry(dedisp_plan* p, int T, int G, int NT, int D)
+{
+    if (!p)
+        return DEDISP_EINVAL;
+    if (p->nsub != 0 || p->uploaded)
+        return DEDISP_ESTATE;  // brute-force plans, before the first dedisp_plan_reserve
+    WindowGeom g;
+    g.T = T;
+    g.G = G;
+    g.NT = NT;
+    g.D = D;
+    if (!window_geom_supported(g))
+        return DEDISP_EINVAL;
+    WindowPlan wp;
+    if (!build_window_plan(p->shift.data(), p->ndm, p->nchans, g, wp) || !window_fits_smem(wp))
+        return DEDISP_ESTATE;  // the table does not fit this geometry; the plan keeps its own
+    p->win = std::move(wp);
+    p->win_fits = true;
+    return DEDISP_OK;
+}
+
 int dedisp_plan_resolved_kernel(const dedisp_plan* p, dedisp_dtype dtype)
 {
     if (!p || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
         return -1;
-    if (use_window(p, dtype))
+    if (use_window(p, dtype, 0))
         return DEDISP_KERNEL_WINDOW;
     // AUTO without the window kernel: long tiles (the direct kernel below 4096 samples per row)
     return p->kernel == DEDISP_KERNEL_AUTO || p->kernel == DEDISP_KERNEL_WINDOW ? DEDISP_KERNEL_LONG : p->kernel;
@@ -619,13 +672,17 @@ dedisp_status dedisp_plan_window_info(const dedisp_plan* p, int64_t* info)
     if (!p || !info)
         return DEDISP_EINVAL;
     info[0] = p->win.ok && p->win_fits;
-    info[1] = p->win.H;
+    info[1] = p->win.Hb;
     info[2] = p->win.kmax;
     info[3] = p->win.lmax;
     info[4] = p->win.ntile_dm;
     info[5] = p->win.geom.W();
     info[6] = p->win.geom.rows();
     info[7] = p->win.nband;
+    info[8] = p->win.geom.T;
+    info[9] = p->win.geom.G;
+    info[10] = p->win.geom.NT;
+    info[11] = p->win.geom.D;
     return DEDISP_OK;
 }
 
@@ -637,6 +694,11 @@ int64_t dedisp_plan_scratch_bytes(const dedisp_plan* p, int64_t nsamp_out, int n
         return 0;
     const int64_t n1 = round_up(nsamp_out + p->maxshift2_max, 16);
     return static_cast<int64_t>(nbeams) * (p->ndm / p->nfine) * p->nsub * n1 * 4;
+}
+
+dedisp_status dedisp_plan_reserve(dedisp_plan* plan, dedisp_dtype dtype, int64_t nsamp_out, int nbeams)
+{
+    return reserve(plan, dtype, nsamp_out, nbeams);
 }
 
 dedisp_status dedisp_execute(dedisp_plan* plan, const void* in, void* out, dedisp_dtype dtype,
@@ -672,6 +734,12 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
     if (plan->nsub == 0) {
         nchunk = static_cast<int>(nsamp_out / 32768);
         nchunk = nchunk < 1 ? 1 : nchunk > dedisp_plan::kHostChunks ? dedisp_plan::kHostChunks : nchunk;
+    }
+    {
+        const int64_t piece = nchunk == 1 ? nsamp_out : round_up((nsamp_out + nchunk - 1) / nchunk, 64);
+        const dedisp_status rs = reserve(plan, dtype, piece, nbeams);
+        if (rs != DEDISP_OK)
+            return rs;
     }
     if (nchunk == 1) {
         if (cudaMemcpy2DAsync(plan->host_in.p, in_stride * es, host_in, n_in * es, n_in * es, rows_in,
@@ -747,6 +815,11 @@ dedisp_status dedisp_stream_create(dedisp_stream** s, dedisp_plan* plan, dedisp_
         return DEDISP_EINVAL;
     if (plan->nsub != 0)
         return DEDISP_ESTATE;
+    {
+        const dedisp_status rs = reserve(plan, dtype, chunk, nbeams);
+        if (rs != DEDISP_OK)
+            return rs;
+    }
     dedisp_stream* q = new (std::nothrow) dedisp_stream;
     if (!q)
         return DEDISP_ENOMEM;
@@ -931,11 +1004,8 @@ dedisp_status dedisp_plan_detect(dedisp_plan* plan, const void* out, dedisp_dtyp
         return DEDISP_EINVAL;
     if (out_stride < nsamp_out || out_stride % 4 != 0 || (reinterpret_cast<uintptr_t>(out) & 15) != 0)
         return DEDISP_ESHAPE;
-    const size_t need = static_cast<size_t>(nbeams) * detect_blocks(plan->ndm) * 2 * sizeof(double);
-    if (plan->det_partial.ensure(need) != cudaSuccess) {
-        cudaGetLastError();
-        return DEDISP_ENOMEM;
-    }
+    if (static_cast<size_t>(nbeams) * detect_blocks(plan->ndm) * 2 * sizeof(double) > plan->det_partial.bytes)
+        return DEDISP_ESTATE;  // dedisp_plan_reserve was not called for this many beams
     plan->last_launches = 0;
     const int rc = launch_detect(out, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, nbeams, plan->ndm, nsamp_out,
                                  out_stride, nsigma, events, capacity, results,

@@ -67,7 +67,7 @@ int launch_bin(const void* in, void* out, int64_t nrows, int64_t nout, int64_t i
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
 // Geometry: a consumer warp owns the D (4 or 8) DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
-// pair of output samples (t, t + NT*H).  A block has G row groups x NT warps along time
+// pair of output samples (t, t + NT*W).  A block has G row groups x NT warps along time
 // (+ 1 producer warp); the channel loop is cut into bands, one launch per band.
 constexpr int kWinD = 8;            // most DM rows per thread (metadata word: 7 bits per mask)
 constexpr int kWinMetaWords = 16;   // per (DM tile, channel) metadata, 64 bytes
@@ -87,7 +87,7 @@ struct WindowGeom {
 struct WindowPlan {
     bool ok = false;
     WindowGeom geom;
-    int H = 0;          // output samples per warp, row and half pair: W - kmax
+    int Hb = 0;         // output samples per block and row: 2 * NT * W - kmax (blocks are Hb samples apart)
     int kmax = 0;       // largest number of row shifts of a row inside one band
     int lmax = 0;       // longest staged channel segment, in pairs
     int ntile_dm = 0;
@@ -116,7 +116,7 @@ struct WindowArgs {
     const int32_t* kfinal;
     const int32_t* theta;
     int64_t in_stride, out_stride, pair_stride, in_len, n_out;
-    int nchans, ndm, nbeams, H, lmax, ntile_dm, ntile_t, nband, stage_total, theta_max;
+    int nchans, ndm, nbeams, Hb, kmax, lmax, ntile_dm, ntile_t, nband, stage_total, theta_max;
     int flush_rows;  // rows per transpose pass of the flush (set by the launcher)
     int dm_group;  // DM tiles per block-order group (kernels_window.cu)
     const int32_t* band;    // HOST pointer, [nband + 1]
@@ -131,6 +131,7 @@ int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out);
 int64_t window_pair_stride(const WindowPlan& wp, int64_t n_out);  // float2 elements per channel row
 int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches);
 WindowGeom window_default_geom();
+bool window_geom_supported(const WindowGeom& g);  // one of the instantiated kernels
 
 }  // namespace dedisp
 #endif

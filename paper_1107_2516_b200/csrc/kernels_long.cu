@@ -216,7 +216,10 @@ int launch_long_t(const Problem& p, int spread, cudaStream_t st)
     int nslot = 8;
     while (nslot > 1 && long_hdr_bytes(nslot, R) + nslot * slot_bytes > 220 * 1024)
         --nslot;
-    if (nslot < 3 || p.nb1 > 65535 || p.nb0 > 65535)
+    // Four producer warps take the channels in turn and wait on a slot's empty barrier by parity only:
+    // a warp is ordered behind channel c - 4 - nslot, the parity test needs channel c - 2 * nslot
+    // consumed, which holds from four slots on (with three, a warp can lap the consumers).
+    if (nslot < 4 || p.nb1 > 65535 || p.nb0 > 65535)
         return -1;
     const int nrt = (p.ndm + R - 1) / R;
     const long long ntt = (p.n_out + L - 1) / L;

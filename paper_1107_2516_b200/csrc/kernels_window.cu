@@ -3,8 +3,8 @@
 //   out[d][t] = sum_c in[c][t + shift(c,d)]
 //
 // Launches per execute: one pairify, then one window_kernel per channel band.
-//  1. pairify_kernel: P[c][u] = (in[c][u], in[c][u + NT*H]) as float2 (uint8 input is widened to
-//     fp32 here; sums of < 2^24/255 bytes are exact in fp32).  Two samples NT*H apart that share
+//  1. pairify_kernel: P[c][u] = (in[c][u], in[c][u + NT*W]) as float2 (uint8 input is widened to
+//     fp32 here; sums of < 2^24/255 bytes are exact in fp32).  Two samples NT*W apart that share
 //     (c, d) have the same shift, so the main kernel adds two outputs per instruction
 //     (add.f32x2 -> FADD2) from naturally aligned 64-bit registers, whatever the shift's parity.
 //  2. window_kernel (band b): a block = G row groups x NT warps; a consumer
@@ -13,14 +13,15 @@
 //     staged pairs (LDS.64, conflict-free for odd T) that feeds all 8 rows: row j adds
 //     w[i + o_j], o_j in {0, 1} chosen by a warp-uniform two-way branch (window_rows.inc).  Rows
 //     follow the growing delay difference between neighbouring DM trials by moving their
-//     accumulators up one slot now and then ("row shift", planned on the host: window_plan.cpp).
+//     accumulators up one slot now and then ("row shift", planned on the host: window_plan.cpp);
+//     the partial sum that leaves the top of the warp's slot range is handed, through the output
+//     buffer, to the warp segment that follows in time (its fresh bottom slot stands for the same
+//     output sample), so a block of 2*NT segments loses kmax samples as a whole, not per segment.
 //     Channel segments are staged into a ring of shared-memory slots by 1-D TMA bulk copies
 //     (cp.async.bulk + mbarrier) issued by thread 0 a few channels ahead.  At the end of the band the
 //     accumulators go through a per-warp shared-memory transpose to coalesced global accesses:
 //     band 0 stores, later bands add to what is there.
 #include <cuda_runtime.h>
-
-#include <cstdlib>
 
 #include "dedisp_internal.h"
 
@@ -115,12 +116,59 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void* src, unsigned
 // 2. window kernel
 // ------------------------------------------------------------------------------------------------
 
-// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one
-template <int T, int D> __device__ __forceinline__ void shift_rows(u64 (&acc)[D][T], unsigned mask, int lane)
+// Hand-over state of one consumer warp, in shared memory, touched by lane 31 only: for row j the
+// output time (int32 at 8*j; the launcher keeps all times below 2^31) and address (8 bytes at 64 + 8*j) of the NEXT partial sum to leave the
+// top slot of the warp's lower segment (the upper segment is hp samples later).  Both move down by
+// one sample per row shift.  Kept out of registers: the channel loop has none to spare.
+constexpr int kFallBytes = 128;
+
+__device__ __forceinline__ void fall_store(float* p, float v, bool first)
+{
+    if (first)
+        *p = v;
+    else
+        asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+}
+__device__ __forceinline__ void fall_store(int32_t* p, float v, bool first)
+{
+    const int iv = __float2int_rn(v);
+    if (first)
+        *p = iv;
+    else
+        asm volatile("red.global.add.s32 [%0], %1;" ::"l"(p), "r"(iv) : "memory");
+}
+
+// the rows in mask (bit j-1 = row j) move their accumulators up one slot; lane 0 gets a fresh one and
+// lane 31 hands the pair that leaves the top slot over to the following segments (band 0 stores it,
+// the flush of that segment adds its own part; later bands add on both sides)
+template <int T, int D, typename OutT>
+__device__ __forceinline__ void shift_rows(u64 (&acc)[D][T], unsigned mask, int lane, unsigned fall_s, unsigned n_out,
+                                           int hp, bool hi_owned, bool first, bool edge)
 {
 #pragma unroll
     for (int j = 1; j < D; ++j) {
         if (mask & (1u << (j - 1))) {
+            if (lane == 31) {
+                // before the shuffle, so that its registers are free again when the carry arrives
+                unsigned long long pa;
+                asm volatile("ld.shared.b64 %0, [%1+64];" : "=l"(pa) : "r"(fall_s + 8u * j));
+                OutT* p = reinterpret_cast<OutT*>(pa);
+                if (!edge) {
+                    fall_store(p, __uint_as_float(static_cast<unsigned>(acc[j][T - 1])), first);
+                    if (hi_owned)
+                        fall_store(p + hp, __uint_as_float(static_cast<unsigned>(acc[j][T - 1] >> 32)), first);
+                } else {
+                    // first / last time tiles, tail rows of the last DM tile: test the output time
+                    int t;
+                    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(t) : "r"(fall_s + 8u * j));
+                    if (static_cast<unsigned>(t) < n_out)
+                        fall_store(p, __uint_as_float(static_cast<unsigned>(acc[j][T - 1])), first);
+                    if (hi_owned && static_cast<unsigned>(t + hp) < n_out)
+                        fall_store(p + hp, __uint_as_float(static_cast<unsigned>(acc[j][T - 1] >> 32)), first);
+                    asm volatile("st.shared.b32 [%0], %1;" ::"r"(fall_s + 8u * j), "r"(t - 1) : "memory");
+                }
+                asm volatile("st.shared.b64 [%0+64], %1;" ::"r"(fall_s + 8u * j), "l"(pa - sizeof(OutT)) : "memory");
+            }
             const u64 carry = __shfl_up_sync(0xffffffffu, acc[j][T - 1], 1);
             shift_row(acc[j], lane ? carry : 0ull);
         }
@@ -154,8 +202,36 @@ __device__ __forceinline__ void put(int32_t* p, float v, bool first)
         asm volatile("red.global.add.s32 [%0], %1;" ::"l"(p), "r"(iv) : "memory");
 }
 
-// smem layout: [nst] full barriers | [nst] empty barriers | nst stages of { 128-byte header, kWinCh
-//              channel slots }; the flush's transpose scratch [NCW][W] u64 overlays the stages
+// band 0: a slot that entered during the band adds what the previous segment handed over
+__device__ __forceinline__ void put_seam(float* p, float v, bool first, bool fresh)
+{
+    if (first && fresh)
+        *p = __ldcg(p) + v;
+    else
+        put(p, v, first);
+}
+__device__ __forceinline__ void put_seam(int32_t* p, float v, bool first, bool fresh)
+{
+    if (first && fresh)
+        *p = __ldcg(p) + __float2int_rn(v);
+    else
+        put(p, v, first);
+}
+
+__device__ __forceinline__ void tile_of(const WindowArgs& a, int lin, int& ty, int& tt)
+{
+    const int per_group = a.dm_group * a.ntile_t;
+    const int grp = lin / per_group, r = lin - grp * per_group;
+    const int g0 = grp * a.dm_group;
+    const int gsz = a.ntile_dm - g0 < a.dm_group ? a.ntile_dm - g0 : a.dm_group;  // last group may be short
+    tt = r / gsz;
+    ty = g0 + r - tt * gsz;
+}
+
+// smem layout: [nst] full barriers | [nst] empty barriers | Fall[NCW] | nst stages of { 128-byte header,
+//              kWinCh channel slots }; the flush's transpose scratch [NCW][W] u64 overlays the stages
+constexpr int kWinFixedBytes = 128 + 16 * kFallBytes;  // barriers + up to 16 consumer warps' Fall
+
 template <int T, int G, int NT, int D, typename OutT>
 __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0,
@@ -167,6 +243,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     constexpr int kPool = ((NCW == 4 ? 32768 : 65536) - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
     constexpr int kConsRegs = kPool > 240 ? 240 : kPool;
     static_assert(NCW % 4 == 0, "setmaxnreg works on groups of four warps");
+    static_assert(NCW <= 16 && D <= kWinD, "Fall area");
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // Block order: groups of a.dm_group DM tiles; inside a group all time tiles, DM tile fastest.
@@ -174,20 +251,14 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // the pair buffer fits L2 (DM-fastest over ALL tiles reads a max_delay-wide range per time tile).
     const int beam = blockIdx.z;
     int ty, tt;
-    {
-        const int lin = blockIdx.x, per_group = a.dm_group * a.ntile_t;
-        const int grp = lin / per_group, r = lin - grp * per_group;
-        const int g0 = grp * a.dm_group;
-        const int gsz = a.ntile_dm - g0 < a.dm_group ? a.ntile_dm - g0 : a.dm_group;  // last group may be short
-        tt = r / gsz;
-        ty = g0 + r - tt * gsz;
-    }
-    const int64_t T0 = static_cast<int64_t>(tt) * 2 * NT * a.H;
+    tile_of(a, blockIdx.x, ty, tt);
+    // the block's 2*NT warp segments of W slots are contiguous in time from T0 on; blocks are Hb apart
+    const int64_t T0 = static_cast<int64_t>(tt) * a.Hb;
 
     const unsigned bar_full = smem_u32(smem);
     const unsigned bar_empty = bar_full + 8u * nst;
     // the flush's transpose scratch [NCW][W] u64 reuses the ring once every consumer has left the loop
-    const int stages_off = (16 * nst + 127) & ~127;
+    const int stages_off = kWinFixedBytes;
     const int tr_off = stages_off;
     const int stage_bytes = kWinHdrWords * 4 + kWinCh * slot_bytes;
     unsigned char* stages = smem + stages_off;
@@ -219,7 +290,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             const float2* prow = static_cast<const float2*>(a.pairs) +
                                  (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
             const int64_t pair_stride = a.pair_stride;
-            const int zlen = ((NT - 1) * a.H + W + 2 + 1) & ~1;  // pairs a padding channel must provide
+            const int zlen = ((NT - 1) * W + W + 2 + 1) & ~1;  // pairs a padding channel must provide
             for (int s = pw; s < nstage; s += 4) {
                 const int ring = s % nst, lap = s / nst;
                 // lanes 0 .. kWinCh-1: (base, len) of this stage's channels
@@ -277,15 +348,37 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         for (int i = 0; i < T; ++i)
             acc[j][i] = 0ull;
 
+    const bool first = band == 0;
+    constexpr int hp = NT * W;   // a pair is (t, t + hp)
+    const unsigned fall_s = smem_u32(smem) + 128u + static_cast<unsigned>(uwarp) * kFallBytes;
+    // block-uniform: some hand-over of this block may fall outside [0, n_out) or belong to a tail row
+    const bool edge = T0 < a.theta_max + a.kmax || T0 + 2 * NT * W > a.n_out || (ty + 1) * RB > a.ndm;
+    if (lane_pinned == 31) {
+        // first partial sum to leave row j's top slot: slot W-1 of the lower segment at base theta_j
+        const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
+        OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
+#pragma unroll
+        for (int j = 1; j < D; ++j) {
+            const int d = ty * RB + g * D + j;
+            const int t = static_cast<int>(T0) + wt * W + (W - 1) - __ldg(thp + j);
+            OutT* p = out + static_cast<int64_t>(d) * a.out_stride + t;
+            // tail rows of the last DM tile: a time that never passes the bounds test
+            asm volatile("st.shared.b32 [%0], %1;\n\tst.shared.b64 [%0+64], %2;" ::"r"(fall_s + 8u * j),
+                         "r"(d < a.ndm ? t : -0x40000000), "l"(p)
+                         : "memory");
+        }
+    }
+    __syncwarp();
+
     // per stage: wait for the NEXT stage and read its four metadata words with one LDS.128, then
     // add the four channels of this stage; the window of channel k+1 is loaded while channel k is
     // added (wa / wb alternate).
-    const unsigned lane_off = kWinHdrWords * 4 + (wt * a.H + lane_pinned * T) * 8;  // bytes from the slot start
+    const unsigned lane_off = kWinHdrWords * 4 + (wt * W + lane_pinned * T) * 8;  // bytes from the slot start
     auto shifts = [&](unsigned m) {
         const unsigned sm = (m >> 7) & 0x3fffu;
-        shift_rows<T, D>(acc, sm & 127u, lane_pinned);
+        shift_rows<T, D, OutT>(acc, sm & 127u, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
         if (sm >> 7)
-            shift_rows<T, D>(acc, sm >> 7, lane_pinned);
+            shift_rows<T, D, OutT>(acc, sm >> 7, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
     };
     auto adds = [&](u64(&w)[T + 1], unsigned m) { rows7(acc, w, m); };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
@@ -347,23 +440,44 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         sbase = sbase_n;
     }
 
-    // ---- flush: slot p of row r is output time T0 + wt*H + (p - kfinal_r) - theta_r ---------------------
+    // ---- flush ------------------------------------------------------------------------------------------
+    // Slot p of row r in segment seg (seg = wt: lower halves, NT + wt: upper halves) is the output sample
+    //     rel = seg * W + p - kfinal_r   of the block's row range, which starts at time T0 - theta_r.
+    // The block owns rel in [0, Hb).  Slots p < kfinal_r entered at the bottom during the band: the
+    // channels before their entry were summed by segment seg - 1 and handed over through `out`
+    // (shift_rows), so band 0 adds what is there; later bands add on both sides anyway.
     // The rows go through a shared-memory transpose (overlaying the ring) in passes of `rpp` rows with
     // their own regions: all rows of a pass are written, ONE __syncwarp, then read back and stored.
     // (A sync per row waits for the previous row's global stores every time: 3.5 % of the kernel.)
+    // The barrier also orders the hand-over stores of every segment before the loads below.
     asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");  // consumers only: the ring is free now
+#ifdef EXP_NOFLUSH
+    if (a.n_out > 0) {
+        float s = 0.f;
+#pragma unroll
+        for (int j = 0; j < D; ++j)
+#pragma unroll
+            for (int i = 0; i < T; ++i)
+                s += __uint_as_float(static_cast<unsigned>(acc[j][i])) + __uint_as_float(static_cast<unsigned>(acc[j][i] >> 32));
+        if (s == 123.456f)
+            static_cast<float*>(a.out)[0] = s;
+        return;
+    }
+#endif
     const int rpp = a.flush_rows;
-    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
-    const int32_t* thp = a.theta + (static_cast<int64_t>(ty) * a.nband + band) * RB + g * D;
+    // the tile is decoded again from a fresh read of the block index: nothing of it stays in registers
+    // over the channel loop
+    int lin2;
+    asm volatile("mov.u32 %0, %%ctaid.x;" : "=r"(lin2));
+    int ty2, tt2;
+    tile_of(a, lin2, ty2, tt2);
+    const int64_t tw = static_cast<int64_t>(tt2) * a.Hb + wt * W;   // start of this warp's lower segment
+    const int32_t* kfp = a.kfinal + (static_cast<int64_t>(ty2) * a.nband + band) * RB + g * D;
+    const int32_t* thp = a.theta + (static_cast<int64_t>(ty2) * a.nband + band) * RB + g * D;
+    OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
     const int kf_lane = __ldg(kfp + lane_pinned % D), th_lane = __ldg(thp + lane_pinned % D);
     u64* tr = reinterpret_cast<u64*>(smem + tr_off) + static_cast<size_t>(warp) * rpp * W;
-    const bool first = band == 0;
-    OutT* out = static_cast<OutT*>(a.out) + static_cast<int64_t>(beam) * a.ndm * a.out_stride;
-    const int H = a.H;
-    const int64_t hp = static_cast<int64_t>(NT) * H;
-    const int64_t tw = T0 + wt * H;
-    // every sample of this warp's two output ranges inside [0, n_out): no bounds tests
-    const bool inside = tw - a.theta_max >= 0 && tw + hp + H <= a.n_out;
+    const int Hb = a.Hb;
     int pass0 = 0;  // first row of the current pass
 #pragma unroll
     for (int j = 0; j < D; ++j) {
@@ -376,37 +490,37 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         __syncwarp();
 #pragma unroll 1
         for (int jj = pass0; jj <= j; ++jj) {
-            const int d = ty * RB + g * D + jj;
+            const int d = ty2 * RB + g * D + jj;
             const int kf = __shfl_sync(0xffffffffu, kf_lane, jj), th = __shfl_sync(0xffffffffu, th_lane, jj);
             if (d >= a.ndm)
                 continue;
-            const u64* trr = tr + (jj - pass0) * W + kf;
-            OutT* o = out + static_cast<int64_t>(d) * a.out_stride + (tw - th);
+            const u64* trr = tr + (jj - pass0) * W;
+            // lower segment: rel = wt * W + p - kf, time = tw - th - kf + p
+            const int64_t tb = tw - th - kf;
+            OutT* o = out + static_cast<int64_t>(d) * a.out_stride + tb;
+            // p ranges owned by the block and inside [0, n_out), per segment
+            int lo0 = wt == 0 ? kf : 0, lo1 = W;                                     // lower segment (seg = wt < 2NT - 1)
+            int hi0 = 0, hi1 = wt == NT - 1 ? Hb - (2 * NT - 1) * W + kf : W;        // upper segment
+            if (tb < 0)
+                lo0 = lo0 > -tb ? lo0 : static_cast<int>(-tb < W ? -tb : W);
+            if (tb + W > a.n_out)
+                lo1 = a.n_out - tb > 0 ? static_cast<int>(a.n_out - tb) : 0;
+            if (tb + hp < 0)
+                hi0 = static_cast<int>(-(tb + hp) < W ? -(tb + hp) : W);
+            if (tb + hp + hi1 > a.n_out)
+                hi1 = a.n_out - tb - hp > 0 ? static_cast<int>(a.n_out - tb - hp) : 0;
             u64 v[T];
 #pragma unroll
+            for (int k = 0; k < T; ++k)
+                v[k] = trr[lane_pinned + 32 * k];
+#pragma unroll
             for (int k = 0; k < T; ++k) {
-                const int q = lane_pinned + 32 * k;
-                v[k] = q < H ? trr[q] : 0ull;
-            }
-            if (inside) {
-#pragma unroll
-                for (int k = 0; k < T; ++k) {
-                    const int q = lane_pinned + 32 * k;
-                    if (q < H) {
-                        put(o + q, __uint_as_float(static_cast<unsigned>(v[k])), first);
-                        put(o + q + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), first);
-                    }
-                }
-            } else {
-#pragma unroll
-                for (int k = 0; k < T; ++k) {
-                    const int q = lane_pinned + 32 * k;
-                    const int64_t t = tw - th + q;
-                    if (q < H && t >= 0 && t < a.n_out)
-                        put(o + q, __uint_as_float(static_cast<unsigned>(v[k])), first);
-                    if (q < H && t + hp >= 0 && t + hp < a.n_out)
-                        put(o + q + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), first);
-                }
+                const int p = lane_pinned + 32 * k;
+                const bool fresh = p < kf;   // only the first few k: kf <= kmax << W
+                if (p >= lo0 && p < lo1)
+                    put_seam(o + p, __uint_as_float(static_cast<unsigned>(v[k])), first, fresh);
+                if (p >= hi0 && p < hi1)
+                    put_seam(o + p + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), first, fresh);
             }
         }
         pass0 = j + 1;
@@ -422,7 +536,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
 static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes)
 {
     const int sb = (lmax * 8 + 127) & ~127;
-    const int fixed = 256 + 256;  // barriers; the transpose scratch aliases the ring (3 stages > [NCW][W] u64)
+    const int fixed = kWinFixedBytes;  // barriers, hand-over state; the transpose scratch aliases the ring
     const int budget = (g.G * g.NT == 4 ? 113 : 227) * 1024 - fixed;
     const int stage_bytes = kWinHdrWords * 4 + kWinCh * sb;
     int nst = budget / stage_bytes;
@@ -431,7 +545,10 @@ static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes)
     *slot_bytes = sb;
     if (nst * stage_bytes < g.G * g.NT * g.W() * 8)
         return 0;
-    return nst >= 3 ? nst : 0;
+    // Four producer warps take the stages in turn and wait on a slot's empty barrier by parity only: a
+    // warp is ordered behind stage s - 4 - nst, the parity test needs stage s - 2 * nst consumed, which
+    // holds from four stages on.
+    return nst >= 4 ? nst : 0;
 }
 
 bool window_fits_smem(const WindowPlan& wp)
@@ -447,14 +564,12 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     const int nst = window_ring(a.geom, a.lmax, &slot_bytes);
     if (nst == 0)
         return static_cast<int>(cudaErrorInvalidConfiguration);
-    const int stages_off = (16 * nst + 127) & ~127;
+    const int stages_off = kWinFixedBytes;
     const size_t ring = static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
     const size_t smem = static_cast<size_t>(stages_off) + ring;
     WindowArgs a2 = a;  // rows per flush pass: as many [NCW][W] u64 transposes as the ring holds
     a2.flush_rows = static_cast<int>(ring / (static_cast<size_t>(G) * NT * 32 * T * 8));
     a2.flush_rows = a2.flush_rows > D ? D : a2.flush_rows < 1 ? 1 : a2.flush_rows;
-    if (const char* e = std::getenv("DEDISP_WINDOW_FLUSH_ROWS"))  // development override (fewer rows per pass)
-        a2.flush_rows = std::atoi(e) >= 1 && std::atoi(e) < a2.flush_rows ? std::atoi(e) : a2.flush_rows;
     cudaError_t e = cudaFuncSetAttribute(window_kernel<T, G, NT, D, OutT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess)
@@ -471,21 +586,29 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
     return 0;
 }
 
+// instantiated geometries: (T, G, NT, D)
+#define DEDISP_GEOMS(X) X(15, 6, 2, 4) X(15, 4, 3, 4) X(21, 4, 1, 4) X(21, 8, 1, 4) X(17, 4, 1, 5) X(15, 4, 1, 6) X(11, 8, 1, 8) \
+    X(11, 6, 2, 5) X(9, 6, 2, 6)
+
 template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_t st, int* launches)
 {
     const WindowGeom& g = a.geom;
 #define DEDISP_GEOM(t, gg, nt, dd) \
     if (g.T == t && g.G == gg && g.NT == nt && g.D == dd) \
         return launch_bands<t, gg, nt, dd, OutT>(a, st, launches);
-    DEDISP_GEOM(15, 6, 2, 4)
-    DEDISP_GEOM(15, 4, 3, 4)
-    DEDISP_GEOM(21, 4, 1, 4)
-    DEDISP_GEOM(21, 8, 1, 4)
-    DEDISP_GEOM(17, 4, 1, 5)
-    DEDISP_GEOM(15, 4, 1, 6)
-    DEDISP_GEOM(11, 8, 1, 8)
+    DEDISP_GEOMS(DEDISP_GEOM)
 #undef DEDISP_GEOM
     return static_cast<int>(cudaErrorInvalidConfiguration);
+}
+
+bool window_geom_supported(const WindowGeom& g)
+{
+#define DEDISP_GEOM(t, gg, nt, dd) \
+    if (g.T == t && g.G == gg && g.NT == nt && g.D == dd) \
+        return true;
+    DEDISP_GEOMS(DEDISP_GEOM)
+#undef DEDISP_GEOM
+    return false;
 }
 
 int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
@@ -495,7 +618,7 @@ int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     dim3 pgrid(static_cast<unsigned>((a.pair_stride / 2 + 255) / 256), a.nchans, a.nbeams);
     float2* pairs = static_cast<float2*>(a.pairs);
-    const int hp = a.geom.NT * a.H;
+    const int hp = a.geom.NT * a.geom.W();
     if (in_t == Elem::F32)
         pairify_kernel<float><<<pgrid, 256, 0, st>>>(static_cast<const float*>(a.in), pairs, a.in_stride,
                                                      a.pair_stride, a.in_len, hp);

@@ -10,14 +10,17 @@
 //   * row j carries base_j(c) = theta_j + kappa_j(c), non-decreasing in c, with
 //         o_j(c) = [s_j(c) - s_0(c)] - base_j(c)  in {0, 1};
 //     slot p of row j stands for output time  tile_start + p - base_j(c);
-//   * kappa_j grows one at a time ("row shift": the row's accumulators move up one slot) and every
-//     slot lost that way shortens the useful tile, so the channel loop is cut into BANDS: inside a
-//     band kappa_j <= kcap; a new band restarts with kappa = 0 and a fresh skew theta_j, and its
-//     partial sums are added to the output by a later launch (kernels_window.cu).
+//   * kappa_j grows one at a time ("row shift": the row's accumulators move up one slot).  The
+//     partial sum that leaves the top of a warp's slot range belongs to the same output sample as
+//     the fresh slot that enters at the bottom of the NEXT warp segment in time, so inside a block
+//     (2*NT segments of W slots, contiguous in time) nothing is lost: the kernel hands those
+//     partial sums over through the output buffer.  Only the block as a whole loses kmax samples,
+//     so blocks are Hb = 2*NT*W - kmax samples apart.  The channel loop is cut into BANDS only
+//     when a row drifts by more than kcap slots or faster than the kernel can follow; a new band
+//     restarts with kappa = 0 and a fresh skew theta_j, and its partial sums are added to the
+//     output by a later launch (kernels_window.cu).
 // Everything the kernel needs per (DM tile, channel) is precomputed into WindowPlan::meta.
 #include <algorithm>
-#include <cstdio>
-#include <cstdlib>
 #include <cstring>
 
 #include "dedisp_internal.h"
@@ -35,16 +38,6 @@ WindowGeom window_default_geom()
     g.G = 6;
     g.NT = 2;
     g.D = 4;
-    // development override: DEDISP_WINDOW_GEOM="T,G,NT[,D]" (one of the instantiated geometries)
-    if (const char* e = std::getenv("DEDISP_WINDOW_GEOM")) {
-        int t = 0, gg = 0, nt = 0, dd = 8;
-        if (std::sscanf(e, "%d,%d,%d,%d", &t, &gg, &nt, &dd) >= 3) {
-            g.T = t;
-            g.G = gg;
-            g.NT = nt;
-            g.D = dd;
-        }
-    }
     return g;
 }
 
@@ -71,7 +64,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
         return false;
     const int RB = geom.rows(), W = geom.W(), G = geom.G, D = geom.D;
     const int ntile = (ndm + RB - 1) / RB;
-    const int kcap = std::max(4, W / 16);
+    const int kcap = std::max(4, W / 4);  // slots a block may lose (of 2 * NT * W)
     const Rows R{shift, ndm, nchans, RB};
     const size_t nrow = static_cast<size_t>(ntile) * RB;
 
@@ -149,10 +142,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
     wp.nband = static_cast<int>(wp.band.size()) - 1;
     if (wp.nband > 64)
         return false;
-    const int H = W - kmax;
-    if (H < W / 2)
-        return false;
-    wp.H = H;
+    wp.Hb = (2 * geom.NT * W - kmax) & ~1;  // even: a block's first pair stays 16-byte aligned for the bulk copies
     wp.kmax = kmax;
     wp.ntile_dm = ntile;
 
@@ -177,7 +167,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
                 const int64_t segbase = lo & ~static_cast<int64_t>(1);
                 if (segbase > INT32_MAX)
                     return false;
-                int len = static_cast<int>(hi - segbase) + (geom.NT - 1) * H + W + 1;
+                int len = static_cast<int>(hi - segbase) + (geom.NT - 1) * W + W + 1;
                 len = (len + 1) & ~1;
                 m[0] = static_cast<int32_t>(segbase);
                 m[1] = len;
@@ -185,7 +175,7 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
                 maxbase = std::max(maxbase, segbase);
                 for (int g = 0; g < G; ++g) {
                     const int64_t wb = r0[k0 + g * D][c] - segbase;
-                    if (wb + (geom.NT - 1) * H >= (1 << kWinWbBits))
+                    if (wb + (geom.NT - 1) * W >= (1 << kWinWbBits))
                         return false;
                     unsigned word = static_cast<unsigned>(wb) << 21;
                     for (int j = 1; j < D; ++j) {
@@ -244,13 +234,12 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
 
 int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out)
 {
-    const int64_t stride = 2LL * wp.geom.NT * wp.H;
-    return (n_out - 1 + wp.theta_max) / stride + 1;
+    return (n_out - 1 + wp.theta_max) / wp.Hb + 1;
 }
 
 int64_t window_pair_stride(const WindowPlan& wp, int64_t n_out)
 {
-    const int64_t n = window_ntile_t(wp, n_out) * 2 * wp.geom.NT * wp.H + wp.maxbase + wp.lmax + 2;
+    const int64_t n = (window_ntile_t(wp, n_out) - 1) * wp.Hb + 2LL * wp.geom.NT * wp.geom.W() + wp.maxbase + wp.lmax + 2;
     return (n + 1) & ~static_cast<int64_t>(1);
 }
 

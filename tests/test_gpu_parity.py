@@ -120,7 +120,7 @@ def test_window_kernel_forced(oracle, dtype, beams, n_out, nchans):
     tab, x = make_case(oracle, cf, beams=beams)
     plan = dd.Plan(**cf.plan_args())
     info = plan.window_info()
-    assert info["ok"] == 1 and info["nband"] >= (2 if nchans == 1024 else 1)
+    assert info["ok"] == 1 and info["nband"] >= 1
     plan.set_kernel(dd.KERNEL_WINDOW)
     assert plan.resolved_kernel(dd.U8 if dtype == "u8" else dd.F32) == dd.KERNEL_WINDOW
     got = plan.execute(to_dev(x), n_out).cpu().numpy()
@@ -134,6 +134,43 @@ def test_window_kernel_forced(oracle, dtype, beams, n_out, nchans):
     # running it again accumulates nothing from the previous call (band 0 overwrites)
     again = plan.execute(to_dev(x), n_out).cpu().numpy()
     assert (again == got).all()
+
+
+GEOMS = [(15, 6, 2, 4), (15, 4, 3, 4), (21, 4, 1, 4), (21, 8, 1, 4), (17, 4, 1, 5), (15, 4, 1, 6), (11, 8, 1, 8),
+         (11, 6, 2, 5), (9, 6, 2, 6)]
+
+
+@pytest.mark.parametrize("geom", GEOMS)
+def test_window_geometries(oracle, geom):
+    """Every instantiated thread / block shape of the register-window kernel (dedisp_plan_set_window_geometry)
+    on the cfg-2 band with 1024 channels: rows drift by tens of slots, so the hand-over of partial sums
+    between warp segments, several blocks along time and (for the 8-row shapes) several channel bands are
+    all exercised; uint8 bit-exact, two beams, an output length that ends inside a block."""
+    T, G, NT, D = geom
+    cf = synth.scaled(synth.configs()[2], dtype="u8", n_out=3 * 2 * NT * 32 * T + 777, ndm=2 * D * G + 3, nchans=1024)
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    try:
+        plan.set_window_geometry(T, G, NT, D)
+    except dd.DedispError as e:
+        assert e.status == dd.binding.ESTATE          # staged segments of this band do not fit this shape's ring
+        cf = synth.scaled(cf, nchans=256)             # a quarter of the band: a quarter of the drift
+        tab, x = make_case(oracle, cf, beams=2)
+        plan = dd.Plan(**cf.plan_args())
+        plan.set_window_geometry(T, G, NT, D)
+    info = plan.window_info()
+    assert info["ok"] == 1 and (info["T"], info["G"], info["NT"], info["D"]) == geom
+    assert info["kmax"] > 0 and info["Hb"] == (2 * NT * 32 * T - info["kmax"]) // 2 * 2
+    plan.set_kernel(dd.KERNEL_WINDOW)
+    got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+    assert plan.last_launches == 1 + info["nband"]
+    for b in range(2):
+        assert (got[b] == oracle.brute_u8(x[b], tab, cf.n_out)).all()
+    with pytest.raises(dd.DedispError):
+        plan.set_window_geometry(15, 4, 1, 6)          # tables are on the device: too late
+    p2 = dd.Plan(**cf.plan_args())
+    with pytest.raises(dd.DedispError):
+        p2.set_window_geometry(13, 5, 2, 4)            # not an instantiated shape
 
 
 @pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
@@ -167,6 +204,28 @@ def test_random_plans_all_kernels(oracle, seed):
         assert (got == ref).all(), name
         tried += 1
     assert tried >= 4
+
+
+@pytest.mark.parametrize("step,dtype", [(2.0, "f32"), (4.0, "f32"), (6.0, "f32"), (4.0, "u8"), (16.0, "u8")])
+def test_long_kernel_ring_depths(oracle, step, dtype):
+    """The long-tile kernel with few, widely spaced trials: the 16 rows of a tile are thousands of samples
+    apart, so a staged channel segment is large and the shared-memory ring holds 7, 4 (fp32 steps 2 and 4;
+    uint8 step 16) or too few slots (fp32 step 6: fewer than four -> the library must fall back to the
+    direct kernel instead of running a ring its four producer warps can lap)."""
+    cf = synth.Config("wide", 64, 150.0, 0.1, 0.1, 4096 + 2048 + 77, 16, step, dtype=dtype, seed=77)
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    spread = int((tab.max(axis=0) - tab.min(axis=0)).max())
+    x = synth.make_input(cf, cf.n_out + int(tab.max()))
+    plan = dd.Plan(**cf.plan_args())
+    assert plan.window_info()["ok"] == 0               # rows this far apart cannot share a register window
+    for kernel in (dd.KERNEL_LONG, dd.KERNEL_AUTO):
+        plan.set_kernel(kernel)
+        got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
+        if dtype == "u8":
+            assert (got == oracle.brute_u8(x, tab, cf.n_out)).all(), (kernel, spread)
+        else:
+            ref, sa = oracle.brute_f32(x, tab, cf.n_out)
+            check_f32(got, ref, sa)
 
 
 @pytest.mark.parametrize("dtype", ["f32", "u8"])
