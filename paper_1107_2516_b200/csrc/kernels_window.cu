@@ -71,14 +71,15 @@ __device__ __forceinline__ void mbar_arrive(unsigned bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive_lane0(unsigned bar, int lane)
+// one lane of the (converged) warp arrives; elect.sync needs no lane id in a register
+__device__ __forceinline__ void mbar_arrive_one(unsigned bar)
 {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "setp.eq.s32 p, %1, 0;\n"
+        "elect.sync _|p, 0xffffffff;\n"
         "@p mbarrier.arrive.shared::cta.b64 _, [%0];\n"
-        "}\n" ::"r"(bar), "r"(lane) : "memory");
+        "}\n" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
 {
@@ -202,21 +203,9 @@ __device__ __forceinline__ void put(int32_t* p, float v, bool first)
         asm volatile("red.global.add.s32 [%0], %1;" ::"l"(p), "r"(iv) : "memory");
 }
 
-// band 0: a slot that entered during the band adds what the previous segment handed over
-__device__ __forceinline__ void put_seam(float* p, float v, bool first, bool fresh)
-{
-    if (first && fresh)
-        *p = __ldcg(p) + v;
-    else
-        put(p, v, first);
-}
-__device__ __forceinline__ void put_seam(int32_t* p, float v, bool first, bool fresh)
-{
-    if (first && fresh)
-        *p = __ldcg(p) + __float2int_rn(v);
-    else
-        put(p, v, first);
-}
+template <typename OutT> __device__ __forceinline__ OutT to_out(float v);
+template <> __device__ __forceinline__ float to_out<float>(float v) { return v; }
+template <> __device__ __forceinline__ int32_t to_out<int32_t>(float v) { return __float2int_rn(v); }
 
 __device__ __forceinline__ void tile_of(const WindowArgs& a, int lin, int& ty, int& tt)
 {
@@ -430,7 +419,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             }
         }
         __syncwarp();
-        mbar_arrive_lane0(bar_empty + 8u * ring, lane_pinned);
+        mbar_arrive_one(bar_empty + 8u * ring);
         if (s + 1 < nstage) {
             mbar_wait(bar_full + 8u * ring_n, par_n);
             mq = *reinterpret_cast<const uint4*>(sbase_n + hdr_off);
@@ -513,14 +502,41 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
 #pragma unroll
             for (int k = 0; k < T; ++k)
                 v[k] = trr[lane_pinned + 32 * k];
+            if (first) {
+                // What the previous segment handed over for the slots that entered during the band (p < kf:
+                // the first KF groups of 32 slots at most) is read first, so that the loads' latency hides
+                // behind the stores of the other slots; everything else is plain predicated stores.
+                constexpr int KF = (W / 4 + 31) / 32 < T ? (W / 4 + 31) / 32 : T;   // kf <= kmax <= W / 4
+                OutT sl[KF], sh[KF];
 #pragma unroll
-            for (int k = 0; k < T; ++k) {
-                const int p = lane_pinned + 32 * k;
-                const bool fresh = p < kf;   // only the first few k: kf <= kmax << W
-                if (p >= lo0 && p < lo1)
-                    put_seam(o + p, __uint_as_float(static_cast<unsigned>(v[k])), first, fresh);
-                if (p >= hi0 && p < hi1)
-                    put_seam(o + p + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), first, fresh);
+                for (int k = 0; k < KF; ++k) {
+                    const int p = lane_pinned + 32 * k;
+                    sl[k] = p < kf && p >= lo0 && p < lo1 ? __ldcg(o + p) : OutT(0);
+                    sh[k] = p < kf && p >= hi0 && p < hi1 ? __ldcg(o + p + hp) : OutT(0);
+                }
+#pragma unroll
+                for (int k = T - 1; k >= 0; --k) {
+                    const int p = lane_pinned + 32 * k;
+                    OutT xl = to_out<OutT>(__uint_as_float(static_cast<unsigned>(v[k])));
+                    OutT xh = to_out<OutT>(__uint_as_float(static_cast<unsigned>(v[k] >> 32)));
+                    if (k < KF) {
+                        xl += sl[k];
+                        xh += sh[k];
+                    }
+                    if (p >= lo0 && p < lo1)
+                        o[p] = xl;
+                    if (p >= hi0 && p < hi1)
+                        o[p + hp] = xh;
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < T; ++k) {
+                    const int p = lane_pinned + 32 * k;
+                    if (p >= lo0 && p < lo1)
+                        put(o + p, __uint_as_float(static_cast<unsigned>(v[k])), false);
+                    if (p >= hi0 && p < hi1)
+                        put(o + p + hp, __uint_as_float(static_cast<unsigned>(v[k] >> 32)), false);
+                }
             }
         }
         pass0 = j + 1;
