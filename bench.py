@@ -2,20 +2,27 @@
 """bench.py -- throughput of the de-dispersion hot path on B200 (one JSON line on stdout).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--impl ours|reference]
+                    [--shard beam|dm] [--no-all-configs] [--no-cpu-baseline] [--no-e2e]
 
 A step is one pass of the hot path over one batch of synthetic filterbank data: for the brute-force
-workloads one dedisp_execute (SURVEY.md §8 rows a2/a3 with the plan's a1 table), for cfg4 the two
+workloads one dedisp_execute (SURVEY.md section 8 rows a2/a3 with the plan's a1 table), for cfg4 the two
 subband stages (a4+a5), for cfg5 one streaming push of all beams (a3+a6).  The default workload is
-BASELINE.json's 4096-DM L-band configuration (cfg3), the one the north-star target is quoted on.
+BASELINE.json's 4096-DM L-band configuration (cfg3), the one the north-star target is quoted on; the
+default run also measures the other four configurations (shorter: `all_configs`) and the register-only
+FP32 add microbenchmark that gives the roofline its measured denominator (`fadd_microbench`).
 
 metric  = DM*sample*channel adds per second (nDM * n_out * nchans * nbeams / t), inputs resident
           in HBM, CUDA events on the launching stream, max over ranks.
 e2e     = same metric through the C ABI's host-buffer entry (pinned host in/out, H2D and D2H inside
-          the timed region).
-roofline: the path is bound by the FP32/INT add pipe (gather-and-add, no tensor cores); peak =
-          SMs * 128 lanes * max SM clock.
-N > 1   : every rank de-disperses its own beam of the same workload (no data-path collective),
-          weak scaling; value is the sum over ranks / max time.
+          the timed region); e2e_events = the same with dedisp_execute_detect_host, which ships the
+          events instead of the de-dispersed buffer.
+roofline: the path is bound by the FP32 add pipe (gather-and-add, no tensor cores); peak =
+          SMs * 128 lanes * max SM clock, peak_measured = the microbenchmark.
+          frac is taken on the whole device step of the window path (pair-forming pre-pass included).
+N > 1   : --shard beam (default): every rank de-disperses its own beam of the same workload, weak
+          scaling.  --shard dm: every rank gets the SAME input and a contiguous slice of the DM list
+          (PAPER.md:74), strong scaling.  No data-path collective either way; value = adds of all
+          ranks / max over ranks of the device time.
 """
 import argparse
 import json
@@ -68,11 +75,7 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), [f.strip() for f in line.split(",")]))
 
-    def stop(self, t0, t1):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.06)
-        self.proc.terminate()
+    def window(self, t0, t1):
         rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.05] or [r for (_, r) in self.rows[-3:]]
         sm, mx, pw, reasons = [], [], [], set()
         for r in rows:
@@ -87,16 +90,30 @@ class ClockSampler:
                 "power_w": float(np.median(pw)) if pw else None, "samples": len(sm),
                 "reasons": sorted(reasons)}
 
-
-def adds_per_step(cf, n_out):
-    return float(cf.ndm) * float(n_out) * float(cf.nchans) * float(cf.nbeams)
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
 
 
 def oracle_sample(cf, budget_adds=3.0e11):
-    """A bounded sample of the workload for the CPU oracle: every s-th DM row, a prefix of the
-    time axis, one beam -- sized to about budget_adds additions."""
+    """A bounded sample of the workload for the CPU oracle: brute-force configs -- every s-th DM row, a
+    prefix of the time axis, one beam; the subband config -- a few whole coarse groups on a prefix of the
+    time axis through the two-stage oracle.  Sized to about budget_adds additions of the metric."""
     from oracle import dedisp_oracle as orc
     orc.build()
+    if cf.nsub:
+        n_out = min(cf.n_out, 16384)
+        ncoarse = cf.ndm // cf.nfine
+        ng = int(min(ncoarse, max(1, budget_adds / (float(n_out) * cf.nchans * cf.nfine))))
+        groups = sorted(set(np.linspace(0, ncoarse - 1, ng).astype(int).tolist()))
+        tab = orc.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list, cf.nsub, cf.nfine)
+        x = synth.make_input(cf, n_out + tab.max_delay)
+        desc = "%d of %d coarse groups x %d of %d samples x %d channels, two-stage subband oracle; adds counted as the metric does (nDM*n_out*nchans)" % (
+            len(groups), ncoarse, n_out, cf.n_out, cf.nchans)
+
+        def run():
+            orc.subband(x, tab, n_out, groups=groups, want_sumabs=False)
+        return run, float(len(groups)) * cf.nfine * n_out * cf.nchans, desc, orc.num_threads()
     n_out = min(cf.n_out, 65536)
     rows = max(1, int(budget_adds / (float(n_out) * cf.nchans)))
     rows = min(rows, cf.ndm)
@@ -139,77 +156,88 @@ def run_reference(args, cf):
     print(json.dumps(line))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel", default="auto", choices=["auto", "naive", "direct", "window", "long"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    cf = synth.configs()[WORKLOADS[args.workload]]
-    if args.impl == "reference":
-        return run_reference(args, cf)
+class Ctx:
+    """What every measurement needs: torch, the binding, rank bookkeeping, peaks, the clock sampler."""
 
-    import torch
-    import torch.distributed as dist
-    import paper_1107_2516_b200 as dd
-    from paper_1107_2516_b200 import build as ddbuild
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if rank == 0:
-        ddbuild.build()
-    if world > 1:
-        dist.barrier()
-    args.warmup = max(args.warmup, 3)
+def fadd_leg(ctx):
+    """Register-only add.f32x2 / add.f32 microbenchmark through the ABI."""
+    dd, pk = ctx.dd, ctx.pk
+    res = {}
+    for name, packed in (("add.f32x2", True), ("add.f32", False)):
+        dd.fadd_microbench(packed, iters=2000, repeats=1)
+        w0 = time.time()
+        ms, adds, nsm = dd.fadd_microbench(packed, iters=20000, repeats=8)
+        w1 = time.time()
+        ck = ctx.sampler.window(w0, w1) if ctx.sampler else {}
+        mhz = ck.get("sm_mhz") or pk["sm_max_mhz"]
+        res[name] = {"ms": ms, "adds": adds, "adds_per_s": adds / (ms * 1e-3),
+                     "adds_per_clk_per_sm": adds / (ms * 1e-3) / (nsm * mhz * 1e6), "sm_mhz": mhz,
+                     "clock_source": "nvidia-smi during the run" if ck.get("sm_mhz") else "clocks.max.sm (no sample)"}
+    best = max(res.values(), key=lambda r: r["adds_per_s"])
+    return {"kernels": res, "peak_measured_adds_per_s": best["adds_per_s"], "nominal_adds_per_clk_per_sm": 128,
+            "how": "dedisp_fadd_microbench: 32 warps per SM, 64 independent fp32 accumulators per thread, 20000 x 8 launches"}
 
-    plan = dd.Plan(**cf.plan_args())
-    plan.set_kernel({"auto": dd.KERNEL_AUTO, "naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT,
-                     "window": dd.KERNEL_WINDOW, "long": dd.KERNEL_LONG}[args.kernel])
-    M = plan.max_delay
+
+def measure(ctx, cf, args, steps, warmup, primary):
+    """One workload: device-resident steps, dominant-kernel timing, e2e, (primary only) the side legs."""
+    torch, dd, dist = ctx.torch, ctx.dd, ctx.dist
+    world, rank, local, pk = ctx.world, ctx.rank, ctx.local, ctx.pk
+    dm_shard = args.shard == "dm" and world > 1
+    dm_list = cf.dm_list
+    lo, hi = 0, cf.ndm
+    if dm_shard:
+        lo, hi = shard.dm_slice(cf.ndm, world, rank, multiple=cf.nfine if cf.nsub else 1)
+        dm_list = dm_list[lo:hi]
+    pa = cf.plan_args()
+    pa["dm_list"] = dm_list
+    plan = dd.Plan(**pa)
+    kern = {"auto": dd.KERNEL_AUTO, "naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT,
+            "window": dd.KERNEL_WINDOW, "long": dd.KERNEL_LONG}[args.kernel]
+    if primary and args.geometry:
+        plan.set_window_geometry(*map(int, args.geometry.split(",")))
+    plan.set_kernel(kern)
+    ndm_local = hi - lo
     n_out = cf.n_out
     streaming = cf.nchunks > 1
+    dtc = dd.U8 if cf.dtype == "u8" else dd.F32
     dt_in = torch.uint8 if cf.dtype == "u8" else torch.float32
     dt_out = torch.int32 if cf.dtype == "u8" else torch.float32
-    full_tab_max = int(plan.shifts().max())
+    nb = cf.nbeams
+    # the input extent is that of the WHOLE DM list (every rank of a DM-sharded run holds the same buffer)
+    full_plan = plan if not dm_shard else dd.Plan(**cf.plan_args())
+    M = full_plan.max_delay
+    full_tab_max = int(full_plan.shifts().max())
+    beam0 = 0 if dm_shard else rank
 
-    # ---- synthetic input, seeded; beam index = rank so that every rank has its own data
+    # ---- synthetic input, seeded
     t_gen = time.time()
     if streaming:
         n_in = n_out                      # one chunk per step; the driver carries the overlap
-        host = np.stack([synth.make_input(cf, n_in, beam=shard.beam_of(rank, cf.nbeams, b)) for b in range(cf.nbeams)])
+        host = np.stack([synth.make_input(cf, n_in, beam=shard.beam_of(beam0, nb, b)) for b in range(nb)])
     else:
         n_in = n_out + max(M, full_tab_max if cf.nsub else 0)
-        if cf.nchans * n_in > (1 << 31):   # cfg4: 9 GB of input -- generate on the device
+        if cf.nchans * n_in > (1 << 31):   # cfg4: 9 GB of input -- generated on the device (seeded torch generator)
             host = None
         else:
-            tab = plan.shifts()
-            pulses = synth.draw_pulses(cf, n_out, beam=rank)
-            host = synth.make_input(cf, n_in, pulses, {p[0]: tab[p[0]] for p in pulses}, beam=rank)[None]
+            tab = full_plan.shifts()
+            pulses = synth.draw_pulses(cf, n_out, beam=beam0)
+            host = synth.make_input(cf, n_in, pulses, {p[0]: tab[p[0]] for p in pulses}, beam=beam0)[None]
     stride = (n_in + 15) // 16 * 16
-    nb = cf.nbeams
     if host is not None:
         x = torch.zeros((nb, cf.nchans, stride), dtype=dt_in, device="cuda")
         x[:, :, :n_in] = torch.from_numpy(host).cuda()
     else:
-        g = torch.Generator(device="cuda").manual_seed(cf.seed + rank)
+        g = torch.Generator(device="cuda").manual_seed(cf.seed + beam0)
         x = torch.empty((nb, cf.nchans, stride), dtype=torch.float32, device="cuda")
         for c0 in range(0, cf.nchans, 256):
             x[:, c0:c0 + 256].normal_(generator=g)
     t_gen = time.time() - t_gen
-    out = torch.empty((nb, cf.ndm, n_out), dtype=dt_out, device="cuda")
-    stream = dd.Stream(plan, dd.U8 if cf.dtype == "u8" else dd.F32, n_out, nb) if streaming else None
+    out = torch.empty((nb, ndm_local, n_out), dtype=dt_out, device="cuda")
+    stream = dd.Stream(plan, dtc, n_out, nb) if streaming else None
     xin = x[:, :, :n_in].contiguous() if streaming else x
+    if not streaming:
+        plan.reserve(dtc, n_out, nb)      # tables and scratch up front: execute itself never allocates
 
     def step():
         if streaming:
@@ -223,101 +251,117 @@ def main():
             dist.barrier()
             torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     launches_per_step = plan.last_launches
     sync_all()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-        time.sleep(0.15)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     sync_all()
     w0 = time.time()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record()
     sync_all()
     w1 = time.time()
     ms = e0.elapsed_time(e1)
-    clocks = sampler.stop(w0, w1) if rank == 0 else None
+    clocks = ctx.sampler.window(w0, w1) if ctx.sampler else None
     ms = shard.max_over_ranks(ms, dist if world > 1 else None, "cuda")
-    ms_step = ms / args.steps
-    adds = adds_per_step(cf, n_out)
-    value = adds * world / (ms_step * 1e-3)
+    ms_step = ms / steps
+    adds_local = float(ndm_local) * float(n_out) * float(cf.nchans) * float(nb)
+    adds_job = shard.sum_over_ranks(adds_local, dist if world > 1 else None, "cuda")
+    value = adds_job / (ms_step * 1e-3)
 
-    # ---- end to end through the host-buffer ABI entry (pinned host buffers)
-    e2e = None
-    if not args.no_e2e and host is not None:
-        hin = torch.from_numpy(np.ascontiguousarray(host[:, :, :n_in])).pin_memory()
-        hout = torch.empty((nb, cf.ndm, n_out), dtype=dt_out).pin_memory()
-        ksteps = max(1, min(args.steps, 3))
+    # ---- end to end through the host-buffer ABI entries (pinned host buffers)
+    e2e, e2e_events = None, None
+    if not args.no_e2e:
+        n_host = n_in if streaming else n_out + plan.max_delay      # the extent this plan's host entry expects
+        if host is not None:
+            hin = torch.from_numpy(np.ascontiguousarray(host[:, :, :n_host])).pin_memory()
+        else:
+            hin = torch.empty((nb, cf.nchans, n_host), dtype=dt_in).pin_memory()
+            hin.copy_(x[:, :, :n_host])
+        hout = torch.empty((nb, ndm_local, n_out), dtype=dt_out).pin_memory()
+        ksteps = max(1, min(steps, 3))
 
         def e2e_step():
             if streaming:
                 stream.push_host(hin, hout)
             else:
                 plan.execute_host(hin, n_out, out=hout)
-        e2e_step()
-        sync_all()
-        t0 = time.perf_counter()
-        for _ in range(ksteps):
-            e2e_step()
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        dt = shard.max_over_ranks(dt, dist if world > 1 else None, "cuda")
-        e2e = {"value": adds * world * ksteps / dt, "unit": UNIT,
+
+        def timed(fn):
+            fn()
+            sync_all()
+            t0 = time.perf_counter()
+            for _ in range(ksteps):
+                fn()
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            return shard.max_over_ranks(dt, dist if world > 1 else None, "cuda")
+        dt = timed(e2e_step)
+        e2e = {"value": adds_job * ksteps / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(hin.numel() * hin.element_size()),
                "d2h_bytes_per_step": int(hout.numel() * hout.element_size()), "steps": ksteps,
-               "ms_per_step": 1e3 * dt / ksteps}
+               "ms_per_step": 1e3 * dt / ksteps, "entry": "dedisp_stream_push_host" if streaming else "dedisp_execute_host"}
+        if not streaming and hasattr(plan, "execute_detect_host"):
+            cap = 1 << 20
+            last = {}
+
+            def ev_step():
+                last["r"] = plan.execute_detect_host(hin, n_out, 5.0, capacity=cap)
+            dt = timed(ev_step)
+            res, evs = last["r"]
+            e2e_events = {"value": adds_job * ksteps / dt, "unit": UNIT, "nsigma": 5.0,
+                          "h2d_bytes_per_step": int(hin.numel() * hin.element_size()),
+                          "d2h_bytes_per_step": int(sum(32 + 16 * min(r["count"], cap) for r in res)),
+                          "events": [r["count"] for r in res], "steps": ksteps, "ms_per_step": 1e3 * dt / ksteps,
+                          "entry": "dedisp_execute_detect_host (events and statistics come back, not the buffer)"}
         del hin, hout
 
     if rank != 0:
-        if world > 1:
-            dist.barrier()
-            dist.destroy_process_group()
-        return
+        return None
 
-    # ---- dominant kernel alone (roofline): CUDA events recorded by the library on the launching
-    # stream around the band launches of the register-window kernel (or all launches of the other
-    # paths), averaged over the same number of steps
+    # ---- dominant kernel alone (roofline): CUDA events recorded by the library on the launching stream
     plan.set_timing(True)
     kms, sms = [], []
-    for _ in range(max(3, min(args.steps, 10))):
+    for _ in range(max(3, min(steps, 10))):
         step()
         kms.append(plan.last_kernel_ms())
-        if cf.nsub:
+        try:
             sms.append(plan.last_stage_ms())
+        except dd.DedispError:
+            pass
     plan.set_timing(False)
     kernel_ms = float(np.mean(kms))
-    resolved = plan.resolved_kernel(dd.U8 if cf.dtype == "u8" else dd.F32)
+    resolved = plan.resolved_kernel(dtc)
     kname = {dd.KERNEL_WINDOW: "dedisp::window_kernel (all band launches of one execute)",
              dd.KERNEL_DIRECT: "dedisp::direct_kernel", dd.KERNEL_NAIVE: "dedisp::naive_kernel",
              dd.KERNEL_LONG: "dedisp::long_kernel"}.get(resolved, "?")
 
-    pk = peaks()
     props = torch.cuda.get_device_properties(local)
     nsm = props.multi_processor_count
     alu_peak = nsm * 128 * pk["sm_max_mhz"] * 1e6          # adds/s
-    traffic = None
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get("%s:%d" % (args.workload, resolved))
+        tj = json.load(open(tpath))
+        traffic = tj.get("%s:%d" % (cf.name.split("_")[0], resolved))
+        traffic_src = "profiles/traffic.json (ncu --set full capture of this kernel, static: not measured in this run)"
     subband = None
+    window_parts = None
     if cf.nsub:
         # the two-stage path executes far fewer adds than the brute-force-equivalent count `value`
         # is quoted in: stage 1 = sum_{k,s} (n_out + maxshift2_{k,s}) * nchans/nsub, stage 2 = ndm * n_out * nsub.
         # Stage 1 (the dominant kernel) has no reuse between rows: one shared-memory word per add,
         # so its ceiling is the 128 B/clk/SM shared-memory pipe = a quarter of the add pipe.
-        # stage 1 forms n_out + max_{d in group k} s2(d, s) samples of subband s in group k (what stage 2 reads)
         s2tab = plan.subband_shifts()[1].astype(np.float64)
-        mks = s2tab.reshape(cf.ndm // cf.nfine, cf.nfine, cf.nsub).max(axis=1)          # [ncoarse][nsub]
+        mks = s2tab.reshape(ndm_local // cf.nfine, cf.nfine, cf.nsub).max(axis=1)          # [ncoarse][nsub]
         s1_samples = float((n_out + mks).sum())                                          # per channel of a subband
         s1_adds = float(nb) * s1_samples * (cf.nchans // cf.nsub)
-        s2_adds = float(nb) * cf.ndm * float(n_out) * cf.nsub
+        s2_adds = float(nb) * ndm_local * float(n_out) * cf.nsub
         s1_ms, s2_ms = (float(np.mean([v[k] for v in sms])) for k in (0, 1))
-        s2_bytes = float(nb) * (s1_samples * 4 + float(cf.ndm) * n_out * 4)
+        s2_bytes = float(nb) * (s1_samples * 4 + float(ndm_local) * n_out * 4)
         smem_peak = nsm * 32 * pk["sm_max_mhz"] * 1e6
         kernel_adds, kernel_ms_dom = s1_adds, s1_ms
         kname = "%s (subband stage 1)" % kname
@@ -328,100 +372,184 @@ def main():
                    "stage2_hbm": {"algorithmic_bytes": s2_bytes, "achieved_gbs": s2_bytes / (s2_ms * 1e-3) / 1e9,
                                   "peak_gbs": pk["hbm_gbs"], "frac": s2_bytes / (s2_ms * 1e-3) / 1e9 / pk["hbm_gbs"]}}
     else:
-        kernel_adds, kernel_ms_dom = adds, kernel_ms
+        kernel_adds, kernel_ms_dom = adds_local, kernel_ms
+        if resolved == dd.KERNEL_WINDOW and sms:
+            window_parts = {"pairify_ms": float(np.mean([v[0] for v in sms])), "bands_ms": float(np.mean([v[1] for v in sms]))}
     per_gpu = kernel_adds / (kernel_ms_dom * 1e-3)
     roof = {"bound": "alu", "achieved": per_gpu / 1e12, "peak": alu_peak / 1e12, "unit": "TFLOP/s",
-            "frac": per_gpu / alu_peak, "traffic": traffic,
+            "frac": per_gpu / alu_peak, "traffic": traffic, "traffic_source": traffic_src,
             "peak_how": "%d SMs x 128 FP32 lanes x %.0f MHz (1 add = 1 flop; DESIGN.md section 6)" % (nsm, pk["sm_max_mhz"]),
             "kernel": kname, "kernel_ms": kernel_ms_dom, "algorithmic_adds": kernel_adds,
             "frac_of_step": kernel_ms_dom / ms_step,
+            "frac_on_step": (kernel_adds / (ms_step * 1e-3)) / alu_peak if not cf.nsub else None,
             "frac_at_observed_clock": (per_gpu / (nsm * 128 * clocks["sm_mhz"] * 1e6)
-                                       if clocks and clocks.get("sm_mhz") else None)}
+                                       if clocks and clocks.get("sm_mhz") else None),
+            "timed": "all launches of one execute (window path: pair-forming pre-pass + band launches)" if not cf.nsub else "stage 1 launch",
+            "window_parts": window_parts}
+    if ctx.fadd:
+        roof["peak_measured"] = ctx.fadd["peak_measured_adds_per_s"] / 1e12
+        roof["frac_of_measured"] = per_gpu / ctx.fadd["peak_measured_adds_per_s"]
     in_bytes = float(nb) * cf.nchans * n_in * (1 if cf.dtype == "u8" else 4)
-    out_bytes = float(nb) * cf.ndm * n_out * 4
+    out_bytes = float(nb) * ndm_local * n_out * 4
     hbm = {"algorithmic_bytes": in_bytes + out_bytes, "achieved_gbs": (in_bytes + out_bytes) / (ms_step * 1e-3) / 1e9,
            "peak_gbs": pk["hbm_gbs"], "frac": (in_bytes + out_bytes) / (ms_step * 1e-3) / 1e9 / pk["hbm_gbs"],
            "peak_src": pk["src"]}
 
-    # ---- event detection on the step's output: HBM-bound, two
-    # passes over out (statistics, threshold scan); timed on its own, not part of the step
-    plan.detect(out, 5.0, capacity=1 << 16)
-    d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    torch.cuda.synchronize()
-    d0.record()
-    for _ in range(5):
-        dres, _ev = plan.detect(out, 5.0, capacity=1 << 16)
-    d1.record()
-    torch.cuda.synchronize()
-    det_ms = d0.elapsed_time(d1) / 5
-    det_bytes = 2.0 * float(nb) * cf.ndm * n_out * 4
-    detect = {"nsigma": 5.0, "ms": det_ms, "events": [r["count"] for r in dres], "algorithmic_bytes": det_bytes,
-              "achieved_gbs": det_bytes / (det_ms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
-              "frac": det_bytes / (det_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
-              "note": "includes the host read-back of 32 bytes of statistics per beam and of the stored events"}
+    res = {"workload": "%s: %d ch, %d DM trials, %d samples%s" % (
+               cf.name, cf.nchans, cf.ndm, n_out, ", %d beams, streaming chunk" % nb if streaming else ""),
+           "value": value, "ms_per_step": ms_step, "steps": steps, "warmup": warmup,
+           "real_time_factor": n_out * cf.t_samp_ms * 1e-3 / (ms_step * 1e-3),
+           "dtype": "i32" if cf.dtype == "u8" else "f32",
+           "nchans": cf.nchans, "ndm": cf.ndm, "ndm_this_rank": ndm_local, "n_out": n_out, "nbeams": nb, "max_delay": M,
+           "resolved_kernel": resolved, "window": plan.window_info() if not cf.nsub else None,
+           "l2": "inputs larger than L2 (%.2f GB in, %.2f GB out per step)" % (in_bytes / 1e9, out_bytes / 1e9)
+                 if in_bytes + out_bytes > 126e6 else "L2 flushed by nothing: %.1f MB in + out fit the 126 MB L2 (cfg1 is a parity case, timed for completeness)" % ((in_bytes + out_bytes) / 1e6),
+           "roofline": roof, "subband": subband, "hbm": hbm, "e2e": e2e, "e2e_events": e2e_events,
+           "gpu_launches": launches_per_step * steps, "clocks": clocks, "input_gen_s": t_gen}
 
-    # ---- power + corner turn: the front-end step that produces the
-    # channel-major layout, on a voltage buffer of up to 2^19 spectra (the paper's buffer) x nchans
-    front = None
-    if cf.dtype == "f32":
-        ns = int(min(n_in, 1 << 19, (1 << 31) // cf.nchans))
-        volt = torch.randn((ns, cf.nchans, 2), dtype=torch.float32, device="cuda")
-        vz = torch.view_as_complex(volt)
-        pw = dd.power_corner_turn(vz)
-        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if primary:
+        # ---- event detection on the step's output: HBM-bound; timed on
+        # its own, not part of the step
+        plan.detect(out, 5.0, capacity=1 << 16)
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
-        f0.record()
+        d0.record()
         for _ in range(5):
-            dd.power_corner_turn(vz, out=pw)
-        f1.record()
+            dres, _ev = plan.detect(out, 5.0, capacity=1 << 16)
+        d1.record()
         torch.cuda.synchronize()
-        fms = f0.elapsed_time(f1) / 5
-        fbytes = 12.0 * ns * cf.nchans
-        front = {"op": "power_corner_turn", "spectra": ns, "nchans": cf.nchans, "ms": fms, "algorithmic_bytes": fbytes,
-                 "achieved_gbs": fbytes / (fms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
-                 "frac": fbytes / (fms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm"}
-        del volt, vz, pw
-        # binning, bin factor 2 on the step's own input
-        bx = x[0]
-        dd.bin_samples(bx, 2)
-        torch.cuda.synchronize()
-        f0.record()
-        for _ in range(5):
+        det_ms = d0.elapsed_time(d1) / 5
+        det_bytes = 2.0 * float(nb) * ndm_local * n_out * 4
+        res["detect"] = {"nsigma": 5.0, "ms": det_ms, "events": [r["count"] for r in dres], "algorithmic_bytes": det_bytes,
+                         "achieved_gbs": det_bytes / (det_ms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
+                         "frac": det_bytes / (det_ms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
+                         "note": "two passes over the buffer; includes the host read-back of 32 bytes of statistics per beam and of the stored events"}
+        # ---- power + corner turn and binning (NEXT-2)
+        if cf.dtype == "f32":
+            ns = int(min(n_in, 1 << 19, (1 << 31) // cf.nchans))
+            volt = torch.randn((ns, cf.nchans, 2), dtype=torch.float32, device="cuda")
+            vz = torch.view_as_complex(volt)
+            pw = dd.power_corner_turn(vz)
+            f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            f0.record()
+            for _ in range(5):
+                dd.power_corner_turn(vz, out=pw)
+            f1.record()
+            torch.cuda.synchronize()
+            fms = f0.elapsed_time(f1) / 5
+            fbytes = 12.0 * ns * cf.nchans
+            front = {"op": "power_corner_turn", "spectra": ns, "nchans": cf.nchans, "ms": fms, "algorithmic_bytes": fbytes,
+                     "achieved_gbs": fbytes / (fms * 1e-3) / 1e9, "peak_gbs": pk["hbm_gbs"],
+                     "frac": fbytes / (fms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm"}
+            del volt, vz, pw
+            bx = x[0]
             dd.bin_samples(bx, 2)
-        f1.record()
-        torch.cuda.synchronize()
-        bms = f0.elapsed_time(f1) / 5
-        bbytes = 6.0 * cf.nchans * float(bx.shape[-1])
-        front["binning"] = {"nb": 2, "ms": bms, "algorithmic_bytes": bbytes, "achieved_gbs": bbytes / (bms * 1e-3) / 1e9,
-                            "frac": bbytes / (bms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
-                            "note": "includes the allocation of the output tensor in the binding"}
+            torch.cuda.synchronize()
+            f0.record()
+            for _ in range(5):
+                dd.bin_samples(bx, 2)
+            f1.record()
+            torch.cuda.synchronize()
+            bms = f0.elapsed_time(f1) / 5
+            bbytes = 6.0 * cf.nchans * float(bx.shape[-1])
+            front["binning"] = {"nb": 2, "ms": bms, "algorithmic_bytes": bbytes, "achieved_gbs": bbytes / (bms * 1e-3) / 1e9,
+                                "frac": bbytes / (bms * 1e-3) / 1e9 / pk["hbm_gbs"], "bound": "hbm",
+                                "note": "includes the allocation of the output tensor in the binding"}
+            res["front_end"] = front
 
-    cpu = None
+    if stream is not None:
+        stream.close()
+    plan.close()
+    del x, out
+    torch.cuda.empty_cache()
+
     if not args.no_cpu_baseline:
-        run, sadds, desc, cores = oracle_sample(cf)
+        run, sadds, desc, cores = oracle_sample(cf, budget_adds=3.0e11 if primary else 5.0e10)
         t0 = time.perf_counter()
         run()
         dt = time.perf_counter() - t0
-        cpu = {"value": sadds / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
-               "seconds": dt}
+        res["cpu_baseline"] = {"value": sadds / dt, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                               "seconds": dt}
+    else:
+        res["cpu_baseline"] = None
+    return res
 
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "i32" if cf.dtype == "u8" else "f32", "data": "synthetic",
-            "config": {"workload": "%s: %d ch, %d DM trials, %d samples%s" % (
-                           cf.name, cf.nchans, cf.ndm, n_out,
-                           ", %d beams, streaming chunk" % nb if streaming else ""),
-                       "nchans": cf.nchans, "ndm": cf.ndm, "n_out": n_out, "nbeams": nb,
-                       "max_delay": M, "kernel": args.kernel, "resolved_kernel": plan.resolved_kernel(dd.U8 if cf.dtype == "u8" else dd.F32),
-                       "window": plan.window_info() if not cf.nsub else None,
-                       "l2": "inputs larger than L2 (%.2f GB in, %.2f GB out per step)" % (in_bytes / 1e9, out_bytes / 1e9),
-                       "parallelism": "1 beam per GPU, no collective" if world > 1 else "single GPU"},
-            "real_time_factor": n_out * cf.t_samp_ms * 1e-3 / (ms_step * 1e-3),
-            "roofline": roof, "subband": subband, "hbm": hbm, "detect": detect, "front_end": front, "cpu_baseline": cpu, "e2e": e2e,
-            "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
-            "paper_context": "paper: 50-200x over one Xeon 2.7 GHz core on a Tesla C1060 (PAPER.md:203), ~1.5e10 adds/s",
-            "input_gen_s": t_gen}
-    print(json.dumps(line))
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "naive", "direct", "window", "long"])
+    ap.add_argument("--geometry", default="", help="T,G,NT,D of the register-window kernel (dedisp_plan_set_window_geometry)")
+    ap.add_argument("--shard", default="beam", choices=["beam", "dm"], help="N > 1: one beam per rank (weak) or one DM slice per rank (strong)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true")
+    args = ap.parse_args()
+    cf = synth.configs()[WORKLOADS[args.workload]]
+    if args.impl == "reference":
+        return run_reference(args, cf)
+
+    import torch
+    import torch.distributed as dist
+    import paper_1107_2516_b200 as dd
+    from paper_1107_2516_b200 import build as ddbuild
+
+    ctx = Ctx()
+    ctx.torch, ctx.dd, ctx.dist = torch, dd, dist
+    ctx.world = world = int(os.environ.get("WORLD_SIZE", "1"))
+    ctx.rank = rank = int(os.environ.get("RANK", "0"))
+    ctx.local = local = int(os.environ.get("LOCAL_RANK", "0"))
+    ctx.pk = peaks()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        ddbuild.build()
+    if world > 1:
+        dist.barrier()
+    args.warmup = max(args.warmup, 3)
+    ctx.sampler = None
+    ctx.fadd = None
+    if rank == 0:
+        ctx.sampler = ClockSampler(local)
+        ctx.sampler.start()
+        time.sleep(0.15)
+        ctx.fadd = fadd_leg(ctx)
+
+    res = measure(ctx, cf, args, args.steps, args.warmup, primary=True)
+    others = {}
+    if world == 1 and not args.no_all_configs and args.workload == "cfg3" and args.kernel == "auto":
+        for name in ("cfg1", "cfg2", "cfg4", "cfg5"):
+            r = measure(ctx, synth.configs()[WORKLOADS[name]], args, 5, 3, primary=False)
+            others[name] = r
+
+    if rank == 0:
+        ctx.sampler.stop()
+        line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True,
+                "scaling": "strong" if (args.shard == "dm" and world > 1) else "weak",
+                "vs_baseline": None, "dtype": res["dtype"], "data": "synthetic",
+                "config": {"workload": res["workload"], "nchans": res["nchans"], "ndm": res["ndm"], "n_out": res["n_out"],
+                           "nbeams": res["nbeams"], "max_delay": res["max_delay"], "kernel": args.kernel,
+                           "resolved_kernel": res["resolved_kernel"], "window": res["window"], "l2": res["l2"],
+                           "parallelism": ("single GPU" if world == 1 else
+                                           "%d GPUs, same input, contiguous DM slices (PAPER.md:74), no collective" % world
+                                           if args.shard == "dm" else "%d GPUs, 1 beam per GPU, no collective" % world)},
+                "real_time_factor": res["real_time_factor"], "roofline": res["roofline"], "subband": res["subband"],
+                "hbm": res["hbm"], "detect": res.get("detect"), "front_end": res.get("front_end"),
+                "cpu_baseline": res["cpu_baseline"], "e2e": res["e2e"], "e2e_events": res["e2e_events"],
+                "gpu_launches": res["gpu_launches"], "clocks": res["clocks"], "fadd_microbench": ctx.fadd,
+                "all_configs": others or None,
+                "paper_context": "paper: 50-200x over one Xeon 2.7 GHz core on a Tesla C1060 (PAPER.md:203), ~1.5e10 adds/s",
+                "input_gen_s": res["input_gen_s"]}
+        print(json.dumps(line))
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()

@@ -241,16 +241,17 @@ DEDISP_API int64_t dedisp_plan_max_chunk(const dedisp_plan *plan, dedisp_dtype d
 /* Number of kernels the last execute/push on this plan launched (bench.py's gpu_launches). */
 DEDISP_API int dedisp_plan_last_launches(const dedisp_plan *plan);
 
-/* Timing of the dominant kernel(s) for roofline reports.  With timing on, every execute / push
- * records two CUDA events on the caller's stream: around the band launches of the register-window
- * kernel (its pairify pre-pass excluded) or around all launches of the other paths.
- * dedisp_plan_last_kernel_ms waits for the second event and returns the elapsed milliseconds of the
- * last execute; DEDISP_ESTATE if timing was off.  Off by default (no events, no overhead). */
+/* Timing for roofline reports.  With timing on, every execute / push records CUDA events on the
+ * caller's stream around ALL the kernels it launches (register-window path: the pair-forming pre-pass
+ * and the band launches) and one between its two parts.  dedisp_plan_last_kernel_ms waits for the last
+ * event and returns the elapsed milliseconds of the last execute; DEDISP_ESTATE if timing was off.
+ * Off by default (no events, no overhead). */
 DEDISP_API dedisp_status dedisp_plan_set_timing(dedisp_plan *plan, int on);
 DEDISP_API dedisp_status dedisp_plan_last_kernel_ms(dedisp_plan *plan, float *ms);
-/* Subband plans, timing on: ms[0] = stage 1 (partial sums inside subbands),
- * ms[1] = stage 2 (across subbands) of the last execute; HOST, 2 floats.  DEDISP_ESTATE for
- * brute-force plans or when timing was off. */
+/* The two parts of the last execute, timing on; HOST, 2 floats.  Subband plans: ms[0] = stage 1
+ * (partial sums inside subbands), ms[1] = stage 2 (across subbands).  Brute-force
+ * plans on the register-window kernel: ms[0] = pair-forming pre-pass, ms[1] = band launches.
+ * DEDISP_ESTATE when timing was off or the last execute took another path. */
 DEDISP_API dedisp_status dedisp_plan_last_stage_ms(dedisp_plan *plan, float *ms);
 
 /*
@@ -304,6 +305,22 @@ DEDISP_API dedisp_status dedisp_power_corner_turn(const void *volt, void *out, i
  */
 DEDISP_API dedisp_status dedisp_bin(const void *in, void *out, int64_t nrows, int64_t nsamp, int64_t in_stride,
                                     int64_t out_stride, int nb, void *cuda_stream);
+
+/*
+ * Register-only FP32 add microbenchmark: the measured denominator of the brute-force roofline.  The
+ * method is nchans adds per output sample ("N_c additions"), so its ceiling is the
+ * rate at which the SMs add when no operand comes from memory (nominally
+ * 128 adds per clock and SM).  Launches, on every SM, 32 warps whose threads each add a loop-invariant
+ * operand to 64 independent fp32 accumulators `iters` times -- as 32 packed add.rn.f32x2 (packed != 0:
+ * the instruction the register-window kernel uses) or 64 scalar add.rn.f32 -- `repeats` times after one
+ * warm-up launch, and times them with CUDA events on cuda_stream.
+ *   ms      HOST, elapsed milliseconds of the `repeats` launches
+ *   adds    HOST, fp32 additions they executed
+ *   nsm     HOST or NULL, number of SMs of the current device
+ * Synchronises the stream, allocates 64 bytes for the call.  Errors: DEDISP_EINVAL, DEDISP_ECUDA.
+ */
+DEDISP_API dedisp_status dedisp_fadd_microbench(int packed, int iters, int repeats, float *ms, double *adds, int *nsm,
+                                                void *cuda_stream);
 
 /* Static string for a status code. */
 DEDISP_API const char *dedisp_strerror(dedisp_status status);

@@ -48,6 +48,7 @@ _SIGS = {
     "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
     "dedisp_bin": (_int, [_vp, _vp, _i64, _i64, _i64, _i64, _int, _vp]),
+    "dedisp_fadd_microbench": (_int, [_int, _int, _int, _vp, _vp, _vp, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
 }
@@ -343,6 +344,15 @@ class Stream:
             self.close()
         except Exception:
             pass
+
+
+def fadd_microbench(packed=True, iters=20000, repeats=5, stream=None):
+    """dedisp_fadd_microbench -> (milliseconds, adds executed, number of SMs)."""
+    ms, adds, nsm = ctypes.c_float(0.0), ctypes.c_double(0.0), ctypes.c_int(0)
+    _check(lib().dedisp_fadd_microbench(int(bool(packed)), int(iters), int(repeats), ctypes.addressof(ms),
+                                        ctypes.addressof(adds), ctypes.addressof(nsm), _stream_ptr(stream)),
+           "dedisp_fadd_microbench")
+    return float(ms.value), float(adds.value), int(nsm.value)
 
 
 def version():

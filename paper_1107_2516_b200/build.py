@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdedisp_b200.so")
 SOURCES = ["shift_table.cpp", "window_plan.cpp", "dedisp_api.cu", "kernels_basic.cu", "kernels_long.cu", "kernels_detect.cu", "kernels_front.cu",
-           "kernels_window.cu"]
+           "kernels_microbench.cu", "kernels_window.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fvisibility=hidden", "-cudart", "static"]
 

@@ -227,7 +227,8 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.theta_max = plan->win.theta_max;
     a.ev0 = plan->timing ? plan->ev[0] : nullptr;
     a.ev1 = plan->timing ? plan->ev[1] : nullptr;
-    plan->ev_valid = plan->timing;
+    a.ev_mid = plan->timing ? plan->ev[2] : nullptr;
+    plan->ev_valid = plan->ev_mid_valid = plan->timing;
     a.nband = plan->win.nband;
     a.band = plan->win.band.data();
     a.geom = plan->win.geom;
@@ -298,6 +299,7 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
         (reinterpret_cast<uintptr_t>(out) & 15) != 0)
         return DEDISP_ESHAPE;
     plan->last_launches = 0;
+    plan->ev_mid_valid = false;
     {
         // never allocates, never blocks: tables and scratch come from dedisp_plan_reserve
         int dev = -1;
@@ -576,7 +578,7 @@ dedisp_status dedisp_plan_last_stage_ms(dedisp_plan* p, float* ms)
 {
     if (!p || !ms)
         return DEDISP_EINVAL;
-    if (p->nsub == 0 || !p->ev_valid || !p->ev_mid_valid)
+    if (!p->ev_valid || !p->ev_mid_valid)
         return DEDISP_ESTATE;
     if (cudaEventSynchronize(p->ev[1]) != cudaSuccess ||
         cudaEventElapsedTime(&ms[0], p->ev[0], p->ev[2]) != cudaSuccess ||
@@ -1033,6 +1035,44 @@ dedisp_status dedisp_bin(const void* in, void* out, int64_t nrows, int64_t nsamp
     if (in_stride < nsamp || out_stride < nsamp / nb)
         return DEDISP_ESHAPE;
     return launch_bin(in, out, nrows, nsamp / nb, in_stride, out_stride, nb, cuda_stream) == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+dedisp_status dedisp_fadd_microbench(int packed, int iters, int repeats, float* ms, double* adds, int* nsm_out,
+                                     void* cuda_stream)
+{
+    if (iters <= 0 || repeats <= 0 || !ms || !adds)
+        return DEDISP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, nsm = 0;
+    float* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    bool ok = cudaGetDevice(&dev) == cudaSuccess &&
+              cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess &&
+              cudaMalloc(reinterpret_cast<void**>(&sink), 64) == cudaSuccess && cudaEventCreate(&e0) == cudaSuccess &&
+              cudaEventCreate(&e1) == cudaSuccess;
+    double per_launch = 0.0;
+    if (ok) {
+        ok = launch_fadd_microbench(packed, iters, nsm, sink, st, &per_launch) == 0;  // warm-up launch
+        ok = ok && cudaEventRecord(e0, st) == cudaSuccess;
+        for (int r = 0; r < repeats && ok; ++r)
+            ok = launch_fadd_microbench(packed, iters, nsm, sink, st, &per_launch) == 0;
+        ok = ok && cudaEventRecord(e1, st) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
+             cudaEventElapsedTime(ms, e0, e1) == cudaSuccess;
+    }
+    *adds = per_launch * repeats;
+    if (nsm_out)
+        *nsm_out = nsm;
+    if (e0)
+        cudaEventDestroy(e0);
+    if (e1)
+        cudaEventDestroy(e1);
+    if (sink)
+        cudaFree(sink);
+    if (!ok) {
+        cudaGetLastError();
+        return DEDISP_ECUDA;
+    }
+    return DEDISP_OK;
 }
 
 const char* dedisp_strerror(dedisp_status s)

@@ -64,6 +64,9 @@ int launch_power_corner_turn(const void* volt, void* out, int nchans, int64_t ns
 int launch_bin(const void* in, void* out, int64_t nrows, int64_t nout, int64_t in_stride, int64_t out_stride, int nb,
                void* stream);
 
+// kernels_microbench.cu: register-only FP32 add throughput
+int launch_fadd_microbench(int packed, int iters, int nsm, float* sink, void* stream, double* adds);
+
 // ---- register-window kernel (window_plan.cpp, kernels_window.cu) ---------------------------------
 // Geometry: a consumer warp owns the D (4 or 8) DM rows of one
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
@@ -124,7 +127,7 @@ struct WindowArgs {
     const int32_t* hdr;     // device copy of WindowPlan::hdr
     const void* zeros;      // device, >= lmax pairs of zeros (segments of the padding channels)
     WindowGeom geom;
-    void *ev0, *ev1;  // cudaEvent_t or nullptr: recorded before the first / after the last band launch
+    void *ev0, *ev1, *ev_mid;  // cudaEvent_t or nullptr: before the pair-forming pre-pass, after the last band launch, between the two
 };
 bool window_fits_smem(const WindowPlan& wp);
 int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out);

@@ -635,6 +635,8 @@ int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
     dim3 pgrid(static_cast<unsigned>((a.pair_stride / 2 + 255) / 256), a.nchans, a.nbeams);
     float2* pairs = static_cast<float2*>(a.pairs);
     const int hp = a.geom.NT * a.geom.W();
+    if (a.ev0)
+        cudaEventRecord(static_cast<cudaEvent_t>(a.ev0), st);
     if (in_t == Elem::F32)
         pairify_kernel<float><<<pgrid, 256, 0, st>>>(static_cast<const float*>(a.in), pairs, a.in_stride,
                                                      a.pair_stride, a.in_len, hp);
@@ -645,8 +647,8 @@ int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches)
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess)
         return static_cast<int>(e);
-    if (a.ev0)
-        cudaEventRecord(static_cast<cudaEvent_t>(a.ev0), st);
+    if (a.ev_mid)
+        cudaEventRecord(static_cast<cudaEvent_t>(a.ev_mid), st);
     const int rc = in_t == Elem::F32 ? launch_geom<float>(a, st, launches) : launch_geom<int32_t>(a, st, launches);
     if (a.ev1)
         cudaEventRecord(static_cast<cudaEvent_t>(a.ev1), st);

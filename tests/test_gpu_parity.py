@@ -416,26 +416,38 @@ def test_execute_host_pipelined_chunks(oracle):
         assert (got[b] == ref).all() and (outp[b].numpy() == ref).all()
 
 
-def test_cfg3_full_size_sampled(oracle):
-    """BASELINE cfg 3 at full size in bench.py's launch configuration; 300 outputs sampled over the
-    whole (DM, time) plane are recomputed one by one by the oracle's definition."""
+def pulse_peak_trial(out_rows, d0, t0, w):
+    """argmax over the given DM rows of the boxcar sum over [t0, t0 + w) (P7: SURVEY.md section 8c)."""
+    box = np.asarray(out_rows)[:, t0:t0 + w].astype(np.float64).sum(axis=1)
+    return d0 + int(np.argmax(box)), box
+
+
+def test_cfg3_full_size_every_output(oracle):
+    """BASELINE cfg 3 at full size in bench.py's launch configuration (AUTO = register-window kernel):
+    EVERY one of the 4096 x 262144 outputs against the oracle's triple loop, in slabs of 256 trials
+    (1.1e12 oracle adds, about a minute and a half on the box's 16 cores), then P7 on each of the 10
+    injected pulses: the boxcar sum over the pulse peaks at its own trial (+-1 where the pulse is wider
+    than the sweep difference between neighbouring trials, 10.2 samples at the band bottom)."""
     cf = synth.configs()[3]
     tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
     n_in = cf.n_out + int(tab.max())
     pulses = synth.draw_pulses(cf, cf.n_out)
+    assert len(pulses) == 10
     x = synth.make_input(cf, n_in, pulses, {p[0]: tab[p[0]] for p in pulses})
     plan = dd.Plan(**cf.plan_args())
+    assert plan.resolved_kernel(dd.F32) == dd.KERNEL_WINDOW
     out = plan.execute(to_dev(x), cf.n_out)
-    rng = np.random.default_rng(3)
-    d = np.r_[rng.integers(0, cf.ndm, 280), [0, 0, cf.ndm - 1, cf.ndm - 1] * 5]
-    t = np.r_[rng.integers(0, cf.n_out, 280), [0, cf.n_out - 1] * 10]
-    ref, sa = oracle.brute_samples(x, tab, d, t)
-    got = out[torch.from_numpy(d).cuda(), torch.from_numpy(t).cuda()].cpu().numpy()
-    check_f32(got, ref, sa)
-    # P3-style invariant at full size: DM 0 row is the plain channel sum
-    row0 = out[0].cpu().numpy().astype(np.float64)
-    s0 = x[:, :cf.n_out].sum(axis=0, dtype=np.float64)
-    assert np.abs(row0 - s0).max() <= 1e-5 * np.abs(x[:, :cf.n_out]).sum(axis=0, dtype=np.float64).max()
+    got = out.cpu().numpy()
+    del out
+    torch.cuda.empty_cache()
+    for r0 in range(0, cf.ndm, 256):
+        ref, sa = oracle.brute_f32(x, tab[r0:r0 + 256], cf.n_out)
+        check_f32(got[r0:r0 + 256], ref, sa)
+    for (trial, t0, w, amp) in pulses:
+        lo, hi = max(0, trial - 24), min(cf.ndm, trial + 25)
+        peak, box = pulse_peak_trial(got[lo:hi], lo, t0, w)
+        assert abs(peak - trial) <= 1, (trial, peak, w, amp)
+        assert box[trial - lo] > 0.8 * cf.nchans * amp * w      # nchans * a * w plus noise (P7)
 
 
 def test_cfg2_full_size_every_output(oracle):
@@ -452,57 +464,115 @@ def test_cfg2_full_size_every_output(oracle):
         check_f32(got[r0:r0 + 512], ref, sa)
 
 
-def test_cfg4_full_size_sampled(oracle):
-    """BASELINE cfg 4 at full size in bench.py's launch configuration (9.1 GB of input generated on the
-    device, long-tile kernel for both stages): 200 outputs over the (DM, time) plane recomputed one by
-    one from the oracle's own subband tables; the gather of the 4096 contributing input samples per
-    output is plain indexing on the device tensor, the fp64 sums are the oracle's."""
+def cfg4_pulses(cf):
+    """SURVEY.md section 8d, cfg 4: the 8 drawn pulses, the first 4 moved onto the nominal trial of their
+    coarse group (k*32 + 16), the other 4 onto a group edge (k*32 or k*32 + 31)."""
+    out = []
+    for i, (trial, t0, w, amp) in enumerate(synth.draw_pulses(cf, cf.n_out)):
+        k = trial // cf.nfine
+        out.append((k * cf.nfine + (cf.nfine // 2 if i < 4 else (0 if i % 2 == 0 else cf.nfine - 1)), t0, w, amp))
+    return out
+
+
+def test_cfg4_full_size_seeded(oracle):
+    """BASELINE cfg 4 at full size in bench.py's launch configuration (4096 ch x 555 784 seeded samples =
+    9.1 GB, 32 subbands, 128 coarse x 32 fine trials, long-tile kernel for both stages), with the 8 pulses
+    of the recipe.  (1) every output of coarse groups 0, 1, 64 and 127 against the stage-by-stage subband
+    oracle; (2) P8(i) on the same input: the 128 nominal rows against BRUTE FORCE (oracle.brute_f32);
+    (3) the pulses: those on nominal trials peak at their trial with the brute-force sum, those on group
+    edges keep most of it ("slight sensitivity loss") and never exceed it by more than noise."""
     cf = synth.configs()[4]
     tab = oracle.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list, cf.nsub, cf.nfine)
+    full = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
     plan = dd.Plan(**cf.plan_args())
     assert plan.max_delay == tab.max_delay
-    n_in = cf.n_out + tab.max_delay
+    n_in = cf.n_out + int(full.max())                   # the brute-force extent (>= the two-stage one)
+    pulses = cfg4_pulses(cf)
+    x = synth.make_input(cf, n_in, pulses, {p[0]: full[p[0]] for p in pulses})
     stride = (n_in + 15) // 16 * 16
-    g = torch.Generator(device="cuda").manual_seed(cf.seed)
-    x = torch.empty((cf.nchans, stride), dtype=torch.float32, device="cuda")
-    for c0 in range(0, cf.nchans, 256):
-        x[c0:c0 + 256].normal_(generator=g)
-    out = plan.execute(x[:, :n_in], cf.n_out)
-    rng = np.random.default_rng(4)
-    d = np.r_[rng.integers(0, cf.ndm, 180), [0, 16, cf.ndm - 1, cf.ndm - 32] * 5]
-    t = np.r_[rng.integers(0, cf.n_out, 180), [0, cf.n_out - 1] * 10]
-    idx = oracle.subband_sample_indices(tab, d, t)
-    assert idx.max() < n_in
-    cc = torch.arange(cf.nchans, device="cuda")[None, :].expand(len(d), -1)
-    vals = x[cc, torch.from_numpy(idx).cuda()].cpu().numpy()
-    ref, sa = oracle.sum_samples(vals)
-    got = out[torch.from_numpy(d).cuda(), torch.from_numpy(t).cuda()].cpu().numpy()
-    check_f32(got, ref, sa)
-    del x, out
+    xd = torch.empty((cf.nchans, stride), dtype=torch.float32, device="cuda")
+    for c0 in range(0, cf.nchans, 512):
+        xd[c0:c0 + 512, :n_in] = torch.from_numpy(x[c0:c0 + 512]).cuda()
+    out = plan.execute(xd[:, :n_in], cf.n_out)
+    assert plan.last_launches == 2
+    got = out.cpu().numpy()
+    del out, xd
     torch.cuda.empty_cache()
+    # (1) subband GPU vs subband oracle, every output of four groups
+    for k in (0, 1, 64, 127):
+        ref, sa = oracle.subband(x, tab, cf.n_out, groups=[k])
+        check_f32(got[k * cf.nfine:(k + 1) * cf.nfine], ref, sa)
+    # (2) nominal rows equal brute force (reading R8)
+    nominal = np.arange(tab.ncoarse) * cf.nfine + cf.nfine // 2
+    ref, sa = oracle.brute_f32(x, full[nominal], cf.n_out)
+    check_f32(got[nominal], ref, sa)
+    # (3) pulses
+    for i, (trial, t0, w, amp) in enumerate(pulses):
+        k = trial // cf.nfine
+        bf = oracle.brute_f32(x, full[trial:trial + 1], cf.n_out, want_sumabs=False)[0, t0:t0 + w].sum()
+        lo = k * cf.nfine
+        peak, box = pulse_peak_trial(got[lo:lo + cf.nfine], lo, t0, w)
+        assert bf > 0.9 * cf.nchans * amp * w
+        if i < 4:
+            assert peak == trial and abs(box[trial - lo] - bf) <= 1e-5 * np.abs(x).max() * cf.nchans * w
+        else:
+            # an edge trial is 0.75-0.8 DM units off its group's nominal DM: up to ~70 samples of smear
+            # inside a subband against pulse widths of 40-200 samples
+            ref, sa = oracle.subband(x, tab, cf.n_out, groups=[k])
+            check_f32(got[lo:lo + cf.nfine], ref, sa)
+            assert 0.2 * bf < box[trial - lo] < bf + 6 * np.sqrt(cf.nchans * w)
+    plan.close()
 
 
-def test_cfg5_full_size_streaming_sampled(oracle):
-    """BASELINE cfg 5 at full chunk size (4 beams x 2048 ch x 65536-sample chunks, 3072 trials, uint8):
-    two pushes through the streaming driver; 400 outputs of the second push (which reach back into the
-    first chunk through the carry) recomputed one by one, bit-exact."""
+def test_cfg5_full_size_all_pushes(oracle):
+    """BASELINE cfg 5 at full size: ALL 16 pushes of 4 beams x 2048 ch x 65536 uint8 samples through
+    dedisp_stream_push (3072 trials, max_delay 24 875 carried from chunk to chunk).  Per beam 8 drawn
+    pulses plus 3 placed so that their sweep crosses a chunk boundary.  Beam 0: every 8th DM row over the
+    whole stream, bit-exact against the one-shot oracle (reading R9: the concatenation of the pushes IS the
+    one-shot result); beams 1-3: 400 outputs each, recomputed one by one, spread over all pushes."""
     cf = synth.configs()[5]
     tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
-    M, C, nb = int(tab.max()), cf.n_out, cf.nbeams
-    xs = np.stack([synth.make_input(cf, 2 * C, beam=b) for b in range(nb)])
-    plan = dd.Plan(**cf.plan_args())
-    st = dd.Stream(plan, dd.U8, C, nb)
-    out = torch.empty((nb, cf.ndm, C), dtype=torch.int32, device="cuda")
-    st.push(torch.from_numpy(np.ascontiguousarray(xs[:, :, :C])).cuda(), out)
-    st.push(torch.from_numpy(np.ascontiguousarray(xs[:, :, C:])).cuda(), out)
-    rng = np.random.default_rng(5)
-    d = np.r_[rng.integers(0, cf.ndm, 380), [0, cf.ndm - 1] * 10]
-    tl = np.r_[rng.integers(0, C, 380), [0, C - 1, 0, C - 1] * 5]      # time inside the second push's output
+    M, C, nb, npush = int(tab.max()), cf.n_out, cf.nbeams, cf.nchunks
+    total = npush * C
+    n = total - M                                                # stream times with a full sweep
+    xs = []
     for b in range(nb):
-        ref, _ = oracle.brute_samples(xs[b], tab, d, tl + C - M)       # stream time of output tl of push 1
-        got = out[b][torch.from_numpy(d).cuda(), torch.from_numpy(tl).cuda()].cpu().numpy()
-        assert (got == ref).all()
-    st.close()
+        pulses = synth.draw_pulses(cf, n, beam=b)
+        for k in (3, 7, 12):                                      # sweep of trial 3000 straddles input chunk k
+            pulses.append((3000, k * C - int(tab[3000].max()) // 2, 12, 1.5))
+        xs.append(synth.make_input(cf, total, pulses, {p[0]: tab[p[0]] for p in pulses}, beam=b))
+    rows = np.arange(0, cf.ndm, 8)
+    rng = np.random.default_rng(5)
+    sd = np.r_[rng.integers(0, cf.ndm, 380), [0, cf.ndm - 1] * 10]
+    st_ = np.r_[rng.integers(0, n, 380), [0, n - 1, C - M - 1, C - M] * 5]       # stream times
+    plan = dd.Plan(**cf.plan_args())
+    stream = dd.Stream(plan, dd.U8, C, nb)
+    out = torch.empty((nb, cf.ndm, C), dtype=torch.int32, device="cuda")
+    got0 = np.empty((len(rows), total), dtype=np.int32)
+    gots = np.zeros((nb, len(sd)), dtype=np.int64)
+    rows_d = torch.from_numpy(rows).cuda()
+    for k in range(npush):
+        chunk = np.ascontiguousarray(np.stack([x[:, k * C:(k + 1) * C] for x in xs]))
+        stream.push(torch.from_numpy(chunk).cuda(), out)
+        got0[:, k * C:(k + 1) * C] = out[0][rows_d].cpu().numpy()
+        sel = np.nonzero((st_ + M) // C == k)[0]                  # output (d, t) leaves in push (t + M) // C
+        if len(sel):
+            dd_ = torch.from_numpy(sd[sel]).cuda()
+            tl = torch.from_numpy((st_[sel] + M) - k * C).cuda()
+            for b in range(1, nb):
+                gots[b, sel] = out[b][dd_, tl].cpu().numpy()
+    ref0 = oracle.brute_u8(xs[0], tab[rows], n)
+    assert (got0[:, M:] == ref0).all()
+    for b in range(1, nb):
+        ref, _ = oracle.brute_samples(xs[b], tab, sd, st_)
+        assert (gots[b] == ref).all()
+    # the 3 straddling pulses of beam 0 are recovered at trial 3000 (a row of the checked subset)
+    r3000 = int(np.nonzero(rows == 3000)[0][0])
+    for k in (3, 7, 12):
+        t0 = k * C - int(tab[3000].max()) // 2
+        box = got0[:, M + t0:M + t0 + 12].astype(np.int64).sum(axis=1)
+        assert abs(int(np.argmax(box)) - r3000) <= 1
+    stream.close()
     plan.close()
 
 

@@ -328,6 +328,30 @@ def test_p8_effective_shift_error_bound(oracle):
             assert abs(eff - full[d, c]) <= bound
 
 
+def test_p8_effective_shift_error_cfg4(oracle):
+    """P8(iv) at BASELINE cfg 4's full geometry: the values SURVEY.md section 8c prints for
+    err(c,d) = s1 + s2 - shift(c,d) -- range -67...+72 samples, mean |err| 12.8, per-subband maximum
+    37 (top subband) ... 72 (bottom) -- and the analytic bound |k_c - k_ctop| * |DM_d - D_k| / t_samp + 2."""
+    cf = synth.configs()[4]
+    full = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list).astype(np.int64)
+    tab = oracle.subband_tables(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list, cf.nsub, cf.nfine)
+    cps = cf.nchans // cf.nsub
+    sub = np.arange(cf.nchans) // cps
+    k = np.arange(cf.ndm) // cf.nfine
+    err = tab.s1[k].astype(np.int64) + tab.s2[:, sub].astype(np.int64) - full
+    assert (err.min(), err.max()) == (-67, 72)
+    assert abs(np.abs(err).mean() - 12.8) < 0.05
+    per_sub = np.abs(err).reshape(cf.ndm, cf.nsub, cps).max(axis=(0, 2))
+    assert per_sub[0] == 37 and per_sub[-1] == 72 and (np.diff(per_sub) >= 0).all()
+    # nominal rows: exactly brute force (reading R8)
+    assert (err[np.arange(tab.ncoarse) * cf.nfine + cf.nfine // 2] == 0).all()
+    # analytic bound, channel by channel (delay per unit DM from the oracle's own eq. 1)
+    kc = np.array([oracle.delay_samples(c, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, 1.0) for c in range(cf.nchans)])
+    ddm = np.abs(cf.dm_list - tab.nominal[k])
+    bound = np.ceil(np.abs(kc - kc[sub * cps])[None, :] * ddm[:, None]) + 2
+    assert (np.abs(err) <= bound).all()
+
+
 def test_p8_impulse_through_both_stages(oracle):
     """An impulse at (c0,u0) must land at u0 - s1(c0,k) - s2(d,s(c0)) in every row d."""
     cf, full, tab, x = _sub_case(oracle, 4)
