@@ -280,6 +280,31 @@ DEDISP_API dedisp_status dedisp_plan_detect(dedisp_plan *plan, const void *out, 
                                             dedisp_detect_result *results, void *cuda_stream);
 
 /*
+ * De-dispersion and event detection in one call (PAPER.md:76 is the step right after the hot path).
+ * Arguments as dedisp_execute followed by those of dedisp_plan_detect; `out` still receives the whole
+ * de-dispersed buffer.  For brute-force plans that run on the register-window kernel with a single
+ * channel band, the kernel's flush accumulates the statistics (fp64 sums of x - pivot and (x - pivot)^2,
+ * pivot = sum_c in[c][0], reduced in a fixed order), so detection costs ONE pass over the buffer (the
+ * threshold scan) instead of two; other plans run dedisp_execute followed by dedisp_plan_detect.  Same
+ * definition of mean / sigma / threshold / events either way.  Asynchronous; needs dedisp_plan_reserve.
+ */
+DEDISP_API dedisp_status dedisp_execute_detect(dedisp_plan *plan, const void *in, void *out, dedisp_dtype dtype,
+                                               int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
+                                               double nsigma, dedisp_event *events, int64_t capacity,
+                                               dedisp_detect_result *results, void *cuda_stream);
+/*
+ * Events-only end-to-end entry: HOST input as for dedisp_execute_host, HOST events [nbeams][capacity]
+ * and HOST results [nbeams].  The input goes to the device in time pieces that overlap the kernels, the
+ * de-dispersed buffer stays on the device (plan-owned), and only min(count, capacity) triplets and 32
+ * bytes of statistics per beam come back -- instead of nbeams*ndm*nsamp_out*4 bytes.  Allocates
+ * plan-owned device buffers, synchronises the stream.
+ */
+DEDISP_API dedisp_status dedisp_execute_detect_host(dedisp_plan *plan, const void *host_in, dedisp_dtype dtype,
+                                                    int64_t nsamp_out, int nbeams, double nsigma,
+                                                    dedisp_event *host_events, int64_t capacity,
+                                                    dedisp_detect_result *host_results, void *cuda_stream);
+
+/*
  * Power + corner turn, the two steps before de-dispersion in the paper's real-time pipeline
  * ("(iii) channelizes and calculates total power (iv) transposes data so that it is
  * in channel order"; Table 6).  One fused kernel:

@@ -46,6 +46,8 @@ _SIGS = {
     "dedisp_plan_last_kernel_ms": (_int, [_vp, _vp]),
     "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
     "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
+    "dedisp_execute_detect": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
+    "dedisp_execute_detect_host": (_int, [_vp, _vp, _int, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
     "dedisp_bin": (_int, [_vp, _vp, _i64, _i64, _i64, _i64, _int, _vp]),
     "dedisp_fadd_microbench": (_int, [_int, _int, _int, _vp, _vp, _vp, _vp]),
@@ -247,6 +249,60 @@ class Plan:
         rec = np.dtype([("t", np.int64), ("dm", np.int32), ("value", np.float32)])
         events = [ev[b, :min(int(counts[b]), capacity)].cpu().numpy().view(rec).reshape(-1) for b in range(nb)]
         return results, events
+
+    _REC = np.dtype([("t", np.int64), ("dm", np.int32), ("value", np.float32)])
+
+    def execute_detect(self, x, nsamp_out, nsigma, capacity=1 << 20, out=None, stream=None):
+        """dedisp_execute_detect: de-disperse x (as execute) and detect events in one call.  Returns
+        (out, results, events) with results / events as detect returns them."""
+        import torch
+        if not x.is_cuda:
+            raise RuntimeError("dedisp_execute_detect needs a CUDA tensor (there is no CPU fallback)")
+        dt, odt = _dtype_of(x)
+        x3 = x if x.dim() == 3 else x.unsqueeze(0)
+        nb, nch, _ = x3.shape
+        if nch != self.nchans or x3.stride(2) != 1 or (nb > 1 and x3.stride(0) != nch * x3.stride(1)):
+            raise DedispError(ESHAPE, "dedisp_execute_detect")
+        if out is None:
+            ostride = (int(nsamp_out) + 3) // 4 * 4
+            out3 = torch.empty((nb, self.ndm, ostride), dtype=odt, device=x.device)[:, :, :int(nsamp_out)]
+        else:
+            out3 = out if out.dim() == 3 else out.unsqueeze(0)
+        self._ensure_reserved(dt, int(nsamp_out), int(nb))
+        ev = torch.zeros((nb, capacity, 4), dtype=torch.int32, device=x.device)
+        res = torch.zeros((nb, 4), dtype=torch.float64, device=x.device)
+        _check(lib().dedisp_execute_detect(self._h, x3.data_ptr(), out3.data_ptr(), dt, int(nsamp_out),
+                                           int(x3.stride(1)), int(out3.stride(1)), int(nb), float(nsigma),
+                                           ev.data_ptr(), int(capacity), res.data_ptr(), _stream_ptr(stream)),
+               "dedisp_execute_detect")
+        rh = res.cpu().numpy()
+        counts = rh[:, 3].copy().view(np.int64)
+        results = [dict(mean=float(rh[b, 0]), sigma=float(rh[b, 1]), threshold=float(rh[b, 2]), count=int(counts[b]))
+                   for b in range(nb)]
+        events = [ev[b, :min(int(counts[b]), capacity)].cpu().numpy().view(self._REC).reshape(-1) for b in range(nb)]
+        return (out3 if x.dim() == 3 else out3[0]), results, events
+
+    def execute_detect_host(self, x, nsamp_out, nsigma, capacity=1 << 20, events=None, stream=None):
+        """dedisp_execute_detect_host: x numpy / CPU tensor [nbeams][nchans][nsamp_out+max_delay]; only the
+        events and the statistics come back.  `events`: optional (pinned) CPU tensor / array of
+        nbeams*capacity*16 bytes to receive the triplets.  Returns (results, events)."""
+        xa = x.numpy() if hasattr(x, "numpy") else np.asarray(x)
+        xa = xa if xa.ndim == 3 else xa[None]
+        assert xa.flags.c_contiguous and xa.shape[1] == self.nchans and xa.shape[2] == nsamp_out + self.max_delay
+        dt = F32 if xa.dtype == np.float32 else U8
+        nb = xa.shape[0]
+        if events is None:
+            events = np.zeros((nb, capacity), dtype=self._REC)
+        ea = events.numpy() if hasattr(events, "numpy") else events
+        res = np.zeros((nb, 4), dtype=np.float64)
+        _check(lib().dedisp_execute_detect_host(self._h, xa.ctypes.data, dt, int(nsamp_out), int(nb), float(nsigma),
+                                                ea.ctypes.data, int(capacity), res.ctypes.data, _stream_ptr(stream)),
+               "dedisp_execute_detect_host")
+        counts = res[:, 3].copy().view(np.int64)
+        results = [dict(mean=float(res[b, 0]), sigma=float(res[b, 1]), threshold=float(res[b, 2]), count=int(counts[b]))
+                   for b in range(nb)]
+        ev = ea.view(np.uint8).reshape(nb, -1)[:, :capacity * 16].view(self._REC).reshape(nb, capacity)
+        return results, [ev[b, :min(int(counts[b]), capacity)] for b in range(nb)]
 
     def execute_host(self, x, nsamp_out, out=None, stream=None):
         """x: numpy / CPU tensor [nbeams][nchans][nsamp_out+max_delay] dense; returns numpy out."""

@@ -2,6 +2,7 @@
 // Host-side only; the arithmetic lives in shift_table.cpp (tables) and kernels_*.cu (sums).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -84,7 +85,9 @@ struct dedisp_plan {
     int32_t *d_shift = nullptr, *d_s1 = nullptr, *d_s2 = nullptr, *d_maxshift2 = nullptr, *d_maxshift2_ks = nullptr;
     DevBuf scratch;            // subband intermediate
     DevBuf host_in, host_out;  // staging for dedisp_execute_host
-    DevBuf det_partial;        // dedisp_plan_detect workspace
+    DevBuf det_partial;        // dedisp_plan_detect / dedisp_execute_detect workspace (per-block partial sums)
+    DevBuf det_pivot;          // [nbeams] doubles
+    DevBuf det_events, det_results;  // device staging of dedisp_execute_detect_host
     dedisp_kernel kernel = DEDISP_KERNEL_AUTO;
     int last_launches = 0;
     int nstreams = 0;
@@ -192,6 +195,12 @@ dedisp_status upload(dedisp_plan* p)
     return DEDISP_OK;
 }
 
+bool use_window(const dedisp_plan* p, dedisp_dtype dtype, int64_t nsamp_out);
+bool fused_stats_ok(const dedisp_plan* p, dedisp_dtype dtype, int64_t nsamp_out)
+{
+    return use_window(p, dtype, nsamp_out) && p->win.nband == 1;
+}
+
 bool use_window(const dedisp_plan* p, dedisp_dtype dtype, int64_t nsamp_out)
 {
     if (p->nsub != 0 || !p->win.ok || !p->win_fits)
@@ -205,9 +214,19 @@ bool use_window(const dedisp_plan* p, dedisp_dtype dtype, int64_t nsamp_out)
     return p->kernel == DEDISP_KERNEL_AUTO || p->kernel == DEDISP_KERNEL_WINDOW;
 }
 
+// request to accumulate the outputs' statistics in the register-window kernel's flush
+struct StatReq {
+    const double* pivot;
+    double* partial;
+    int64_t stride, off;  // partials per beam, first partial of this execute
+};
+
+// the fused statistics need every output to be final when it is stored: single-band window plans
+bool fused_stats_ok(const dedisp_plan* p, dedisp_dtype dtype, int64_t nsamp_out);
+
 // brute force through the register-window kernel: pairify into the plan's scratch, then add
 dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t, int64_t nsamp_out,
-                         int64_t in_stride, int64_t out_stride, int nbeams, void* stream)
+                         int64_t in_stride, int64_t out_stride, int nbeams, void* stream, const StatReq* sr)
 {
     WindowArgs a;
     std::memset(&a, 0, sizeof(a));
@@ -228,6 +247,12 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.ev0 = plan->timing ? plan->ev[0] : nullptr;
     a.ev1 = plan->timing ? plan->ev[1] : nullptr;
     a.ev_mid = plan->timing ? plan->ev[2] : nullptr;
+    if (sr) {
+        a.pivot = sr->pivot;
+        a.stat_partial = sr->partial;
+        a.stat_stride = sr->stride;
+        a.stat_off = sr->off;
+    }
     plan->ev_valid = plan->ev_mid_valid = plan->timing;
     a.nband = plan->win.nband;
     a.band = plan->win.band.data();
@@ -283,7 +308,7 @@ int run_problem(dedisp_plan* plan, const Problem& pr, Elem in_t, const int sprea
 
 dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedisp_dtype dtype,
                              int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
-                             void* stream)
+                             void* stream, const StatReq* sr = nullptr)
 {
     if (!plan || nbeams <= 0 || nsamp_out < 0 || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
         return DEDISP_EINVAL;
@@ -314,7 +339,9 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     pr.in_len = nsamp_out + plan->max_delay;  // the extent seen from `in`: nothing beyond it is read
     int rc = 0;
     if (use_window(plan, dtype, nsamp_out))
-        return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream);
+        return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream, sr);
+    if (sr)
+        return DEDISP_ESTATE;  // callers check fused_stats_ok first
     struct Timer {  // the direct / subband kernels are timed as a whole
         dedisp_plan* p;
         cudaStream_t st;
@@ -420,9 +447,12 @@ dedisp_status reserve(dedisp_plan* plan, dedisp_dtype dtype, int64_t nsamp_out, 
     } else {
         scratch = static_cast<size_t>(dedisp_plan_scratch_bytes(plan, nsamp_out, nbeams));
     }
-    const size_t det = static_cast<size_t>(nbeams) * detect_blocks(plan->ndm) * 2 * sizeof(double);
+    size_t npart = static_cast<size_t>(detect_blocks(plan->ndm));
+    if (fused_stats_ok(plan, dtype, nsamp_out) && nsamp_out > 0)
+        npart = std::max(npart, static_cast<size_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nsamp_out));
+    const size_t det = static_cast<size_t>(nbeams) * npart * 2 * sizeof(double);
     if (plan->pairs.ensure(pairs) != cudaSuccess || plan->scratch.ensure(scratch) != cudaSuccess ||
-        plan->det_partial.ensure(det) != cudaSuccess) {
+        plan->det_partial.ensure(det) != cudaSuccess || plan->det_pivot.ensure(nbeams * sizeof(double)) != cudaSuccess) {
         cudaGetLastError();
         return DEDISP_ENOMEM;
     }
@@ -547,6 +577,9 @@ dedisp_status dedisp_plan_destroy(dedisp_plan* p)
     p->host_in.release();
     p->host_out.release();
     p->det_partial.release();
+    p->det_pivot.release();
+    p->det_events.release();
+    p->det_results.release();
     delete p;
     return DEDISP_OK;
 }
@@ -1013,6 +1046,160 @@ dedisp_status dedisp_plan_detect(dedisp_plan* plan, const void* out, dedisp_dtyp
                                  out_stride, nsigma, events, capacity, results,
                                  static_cast<double*>(plan->det_partial.p), cuda_stream, &plan->last_launches);
     return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+dedisp_status dedisp_execute_detect(dedisp_plan* plan, const void* in, void* out, dedisp_dtype dtype, int64_t nsamp_out,
+                                    int64_t in_stride, int64_t out_stride, int nbeams, double nsigma,
+                                    dedisp_event* events, int64_t capacity, dedisp_detect_result* results,
+                                    void* cuda_stream)
+{
+    if (!plan || !results || nsamp_out <= 0 || capacity < 0 || (capacity > 0 && !events) || !(nsigma == nsigma))
+        return DEDISP_EINVAL;
+    if (!fused_stats_ok(plan, dtype, nsamp_out)) {
+        // subband plans, tables outside the window kernel, several channel bands: de-disperse, then the
+        // two-pass detection
+        dedisp_status st = execute_device(plan, in, out, dtype, nsamp_out, in_stride, out_stride, nbeams, cuda_stream);
+        if (st != DEDISP_OK)
+            return st;
+        const int launches = plan->last_launches;
+        st = dedisp_plan_detect(plan, out, dtype, nsamp_out, out_stride, nbeams, nsigma, events, capacity, results,
+                                cuda_stream);
+        plan->last_launches += launches;
+        return st;
+    }
+    const int64_t npart = static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nsamp_out);
+    if (!plan->uploaded || static_cast<size_t>(nbeams) * npart * 2 * sizeof(double) > plan->det_partial.bytes ||
+        static_cast<size_t>(nbeams) * sizeof(double) > plan->det_pivot.bytes)
+        return DEDISP_ESTATE;  // dedisp_plan_reserve was not called for this shape
+    if (!in)
+        return DEDISP_EINVAL;
+    int launches = 0;
+    const Elem in_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::U8;
+    double* pivot = static_cast<double*>(plan->det_pivot.p);
+    if (launch_detect_pivot(in, in_t, nbeams, plan->nchans, in_stride, pivot, cuda_stream, &launches) != 0)
+        return DEDISP_ECUDA;
+    const StatReq sr{pivot, static_cast<double*>(plan->det_partial.p), npart, 0};
+    const dedisp_status st =
+        execute_device(plan, in, out, dtype, nsamp_out, in_stride, out_stride, nbeams, cuda_stream, &sr);
+    if (st != DEDISP_OK)
+        return st;
+    launches += plan->last_launches;
+    const int rc = launch_detect_fused(out, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, nbeams, plan->ndm, nsamp_out,
+                                       out_stride, nsigma, events, capacity, results, sr.partial, npart, npart, pivot,
+                                       cuda_stream, &launches);
+    plan->last_launches = launches;
+    return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in, dedisp_dtype dtype, int64_t nsamp_out,
+                                         int nbeams, double nsigma, dedisp_event* host_events, int64_t capacity,
+                                         dedisp_detect_result* host_results, void* cuda_stream)
+{
+    if (!plan || !host_in || !host_results || nbeams <= 0 || nsamp_out <= 0 || capacity < 0 ||
+        (capacity > 0 && !host_events) || !(nsigma == nsigma) || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t es = in_size(dtype);
+    const int64_t n_in = nsamp_out + plan->max_delay;
+    const int64_t in_stride = round_up(n_in, 16), out_stride = round_up(nsamp_out, 4);
+    const size_t rows_in = static_cast<size_t>(nbeams) * plan->nchans;
+    const size_t rows_out = static_cast<size_t>(nbeams) * plan->ndm;
+    if (plan->host_in.ensure(rows_in * in_stride * es) != cudaSuccess ||
+        plan->host_out.ensure(rows_out * out_stride * 4) != cudaSuccess ||
+        plan->det_events.ensure(static_cast<size_t>(nbeams) * capacity * sizeof(dedisp_event) + 16) != cudaSuccess ||
+        plan->det_results.ensure(static_cast<size_t>(nbeams) * sizeof(dedisp_detect_result)) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    // time pieces as in dedisp_execute_host: the H2D copy of piece i+1 overlaps the kernels of piece i; nothing
+    // but the events and 32 bytes of statistics per beam comes back
+    int nchunk = 1;
+    if (plan->nsub == 0) {
+        nchunk = static_cast<int>(nsamp_out / 32768);
+        nchunk = nchunk < 1 ? 1 : nchunk > dedisp_plan::kHostChunks ? dedisp_plan::kHostChunks : nchunk;
+    }
+    const int64_t csize = nchunk == 1 ? nsamp_out : round_up((nsamp_out + nchunk - 1) / nchunk, 64);
+    dedisp_status rs = reserve(plan, dtype, csize, nbeams);
+    if (rs != DEDISP_OK)
+        return rs;
+    const bool fused = fused_stats_ok(plan, dtype, csize);
+    int64_t npart_total = 0;
+    if (fused) {
+        for (int64_t t0 = 0; t0 < nsamp_out; t0 += csize)
+            npart_total += static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, std::min(csize, nsamp_out - t0));
+        if (plan->det_partial.ensure(static_cast<size_t>(nbeams) * npart_total * 2 * sizeof(double)) != cudaSuccess) {
+            cudaGetLastError();
+            return DEDISP_ENOMEM;
+        }
+    }
+    if (!ensure_copy_streams(plan))
+        return DEDISP_ECUDA;
+    cudaStream_t h2d = plan->copy_st[0];
+    cudaEvent_t* ev_in = plan->ev_copy;
+    cudaEvent_t ev_start = plan->ev_copy[2 * dedisp_plan::kHostChunks];
+    bool ok = cudaEventRecord(ev_start, st) == cudaSuccess && cudaStreamWaitEvent(h2d, ev_start, 0) == cudaSuccess;
+    const char* hin = static_cast<const char*>(host_in);
+    char* din = static_cast<char*>(plan->host_in.p);
+    char* dout = static_cast<char*>(plan->host_out.p);
+    double* pivot = static_cast<double*>(plan->det_pivot.p);
+    const Elem in_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::U8;
+    int launches = 0;
+    int64_t col = 0, part_off = 0;
+    for (int i = 0; i < nchunk && ok; ++i) {
+        const int64_t t0 = i * csize;
+        if (t0 >= nsamp_out)
+            break;
+        const int64_t cn = std::min(csize, nsamp_out - t0);
+        const int64_t need = t0 + cn + plan->max_delay;
+        if (need > col) {
+            ok = cudaMemcpy2DAsync(din + col * es, in_stride * es, hin + col * es, n_in * es, (need - col) * es, rows_in,
+                                   cudaMemcpyHostToDevice, h2d) == cudaSuccess;
+            col = need;
+        }
+        ok = ok && cudaEventRecord(ev_in[i], h2d) == cudaSuccess && cudaStreamWaitEvent(st, ev_in[i], 0) == cudaSuccess;
+        if (!ok)
+            break;
+        if (i == 0 && fused && launch_detect_pivot(din, in_t, nbeams, plan->nchans, in_stride, pivot, cuda_stream, &launches) != 0)
+            return DEDISP_ECUDA;
+        const StatReq sr{pivot, static_cast<double*>(plan->det_partial.p), npart_total, part_off};
+        const dedisp_status s = execute_device(plan, din + t0 * es, dout + t0 * 4, dtype, cn, in_stride, out_stride, nbeams,
+                                               cuda_stream, fused ? &sr : nullptr);
+        if (s != DEDISP_OK)
+            return s;
+        launches += plan->last_launches;
+        part_off += static_cast<int64_t>(plan->win.ntile_dm) * (fused ? window_ntile_t(plan->win, cn) : 0);
+    }
+    if (!ok) {
+        cudaGetLastError();
+        return DEDISP_ECUDA;
+    }
+    dedisp_event* dev = static_cast<dedisp_event*>(plan->det_events.p);
+    dedisp_detect_result* dres = static_cast<dedisp_detect_result*>(plan->det_results.p);
+    const Elem out_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::I32;
+    int rc;
+    if (fused)
+        rc = launch_detect_fused(dout, out_t, nbeams, plan->ndm, nsamp_out, out_stride, nsigma, dev, capacity, dres,
+                                 static_cast<const double*>(plan->det_partial.p), npart_total, npart_total, pivot,
+                                 cuda_stream, &launches);
+    else
+        rc = launch_detect(dout, out_t, nbeams, plan->ndm, nsamp_out, out_stride, nsigma, dev, capacity, dres,
+                           static_cast<double*>(plan->det_partial.p), cuda_stream, &launches);
+    plan->last_launches = launches;
+    if (rc != 0 ||
+        cudaMemcpyAsync(host_results, dres, nbeams * sizeof(dedisp_detect_result), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ECUDA;
+    }
+    for (int b = 0; b < nbeams; ++b) {
+        const int64_t k = std::min<int64_t>(host_results[b].count, capacity);
+        if (k > 0 && cudaMemcpyAsync(host_events + static_cast<int64_t>(b) * capacity, dev + static_cast<int64_t>(b) * capacity,
+                                     k * sizeof(dedisp_event), cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+            cudaGetLastError();
+            return DEDISP_ECUDA;
+        }
+    }
+    return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
 }
 
 dedisp_status dedisp_power_corner_turn(const void* volt, void* out, int nchans, int64_t nsamp, int64_t volt_stride,

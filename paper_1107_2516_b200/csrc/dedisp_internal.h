@@ -57,6 +57,14 @@ int launch_detect(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64
                   dedisp_event* events, int64_t capacity, dedisp_detect_result* res, double* partial, void* stream,
                   int* launches);
 
+// fused variant: pivot[beam] = sum_c in[beam][c][0]; statistics from the partial sums the register-window
+// kernel wrote (WindowArgs::stat_partial), then the threshold scan
+int launch_detect_pivot(const void* in, Elem in_t, int nbeams, int nchans, int64_t chan_stride, double* pivot, void* stream,
+                        int* launches);
+int launch_detect_fused(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64_t stride, double nsigma,
+                        dedisp_event* events, int64_t capacity, dedisp_detect_result* res, const double* partial,
+                        int64_t npart, int64_t part_stride, const double* pivot, void* stream, int* launches);
+
 // kernels_front.cu: out[c][t] = |volt[t][c]|^2, strides in elements
 int launch_power_corner_turn(const void* volt, void* out, int nchans, int64_t nsamp, int64_t volt_stride,
                              int64_t out_stride, void* stream);
@@ -127,6 +135,11 @@ struct WindowArgs {
     const int32_t* hdr;     // device copy of WindowPlan::hdr
     const void* zeros;      // device, >= lmax pairs of zeros (segments of the padding channels)
     WindowGeom geom;
+    // fused statistics of the outputs (band 0 of single-band plans only): per beam a pivot, per block two
+    // fp64 partial sums at stat_partial[(beam * stat_stride + stat_off + block) * 2]; nullptr: off
+    const double* pivot;
+    double* stat_partial;
+    int64_t stat_stride, stat_off;
     void *ev0, *ev1, *ev_mid;  // cudaEvent_t or nullptr: before the pair-forming pre-pass, after the last band launch, between the two
 };
 bool window_fits_smem(const WindowPlan& wp);

@@ -150,6 +150,63 @@ __global__ void __launch_bounds__(kDetThreads) detect_emit_kernel(const T* __res
     }
 }
 
+// ---- fused path (dedisp_execute_detect): the de-dispersion kernel left per-block sums of (x - pivot) and
+// (x - pivot)^2; the pivot is the DM-0 output at t = 0 formed from the input, sum_c in[c][0].
+template <typename InT>
+__global__ void __launch_bounds__(kDetThreads) detect_pivot_kernel(const InT* __restrict__ in, int nchans, int64_t chan_stride,
+                                                                    int64_t beam_stride, double* __restrict__ pivot)
+{
+    __shared__ double part[kDetThreads];
+    const InT* base = in + static_cast<int64_t>(blockIdx.x) * beam_stride;
+    double s = 0.0;
+    for (int c = threadIdx.x; c < nchans; c += kDetThreads)
+        s += static_cast<double>(base[static_cast<int64_t>(c) * chan_stride]);
+    part[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0;
+        for (int k = 0; k < kDetThreads; ++k)
+            a += part[k];
+        pivot[blockIdx.x] = a;
+    }
+}
+
+// one block per beam: thread i adds partials i, i + 256, ... in that order, thread 0 adds the 256 sums in
+// index order -> mean, sigma (population), threshold; cursor = 0.  A fixed order: the statistics do not
+// depend on scheduling.
+__global__ void __launch_bounds__(kDetThreads) detect_finish_fused_kernel(const double* __restrict__ partial, int64_t npart,
+                                                                          int64_t part_stride, const double* __restrict__ pivot,
+                                                                          double count, double nsigma,
+                                                                          dedisp_detect_result* __restrict__ res)
+{
+    __shared__ double p1[kDetThreads], p2[kDetThreads];
+    const double* p = partial + static_cast<int64_t>(blockIdx.x) * part_stride * 2;
+    double a = 0.0, b = 0.0;
+    for (int64_t k = threadIdx.x; k < npart; k += kDetThreads) {
+        a += p[2 * k];
+        b += p[2 * k + 1];
+    }
+    p1[threadIdx.x] = a;
+    p2[threadIdx.x] = b;
+    __syncthreads();
+    if (threadIdx.x != 0)
+        return;
+    a = b = 0.0;
+    for (int k = 0; k < kDetThreads; ++k) {
+        a += p1[k];
+        b += p2[k];
+    }
+    const double m = a / count;
+    double var = b / count - m * m;
+    var = var > 0.0 ? var : 0.0;
+    dedisp_detect_result r;
+    r.mean = pivot[blockIdx.x] + m;
+    r.sigma = sqrt(var);
+    r.threshold = r.mean + nsigma * r.sigma;
+    r.count = 0;
+    res[blockIdx.x] = r;
+}
+
 template <typename T>
 int launch_detect_t(const void* out, int nbeams, int ndm, int64_t n, int64_t stride, double nsigma,
                     dedisp_event* events, int64_t capacity, dedisp_detect_result* res, double* partial, int nblocks,
@@ -166,6 +223,40 @@ int launch_detect_t(const void* out, int nbeams, int ndm, int64_t n, int64_t str
 }
 
 }  // namespace
+
+int launch_detect_pivot(const void* in, Elem in_t, int nbeams, int nchans, int64_t chan_stride, double* pivot, void* stream,
+                        int* launches)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (in_t == Elem::F32)
+        detect_pivot_kernel<float><<<nbeams, kDetThreads, 0, st>>>(static_cast<const float*>(in), nchans, chan_stride,
+                                                                  chan_stride * nchans, pivot);
+    else
+        detect_pivot_kernel<uint8_t><<<nbeams, kDetThreads, 0, st>>>(static_cast<const uint8_t*>(in), nchans, chan_stride,
+                                                                    chan_stride * nchans, pivot);
+    ++*launches;
+    return static_cast<int>(cudaGetLastError());
+}
+
+// finish + threshold scan on statistics the de-dispersion kernel accumulated (two launches, one pass over out)
+int launch_detect_fused(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64_t stride, double nsigma,
+                        dedisp_event* events, int64_t capacity, dedisp_detect_result* res, const double* partial,
+                        int64_t npart, int64_t part_stride, const double* pivot, void* stream, int* launches)
+{
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    detect_finish_fused_kernel<<<nbeams, kDetThreads, 0, st>>>(partial, npart, part_stride, pivot,
+                                                              static_cast<double>(ndm) * n, nsigma, res);
+    dim3 grid(detect_blocks(ndm), nbeams);
+    const int64_t beam_stride = stride * ndm;
+    if (t == Elem::F32)
+        detect_emit_kernel<float><<<grid, kDetThreads, 0, st>>>(static_cast<const float*>(out), ndm, n, stride, beam_stride,
+                                                               res, events, capacity);
+    else
+        detect_emit_kernel<int32_t><<<grid, kDetThreads, 0, st>>>(static_cast<const int32_t*>(out), ndm, n, stride,
+                                                                 beam_stride, res, events, capacity);
+    *launches += 2;
+    return static_cast<int>(cudaGetLastError());
+}
 
 int detect_blocks(int ndm) { return ndm < 1184 ? ndm : 1184; }  // 8 blocks per SM on 148 SMs, whole rows each
 

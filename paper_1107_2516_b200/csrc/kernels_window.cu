@@ -467,6 +467,10 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     const int kf_lane = __ldg(kfp + lane_pinned % D), th_lane = __ldg(thp + lane_pinned % D);
     u64* tr = reinterpret_cast<u64*>(smem + tr_off) + static_cast<size_t>(warp) * rpp * W;
     const int Hb = a.Hb;
+    // fused statistics (dedisp_execute_detect): fp64 sums of (x - pivot) and (x - pivot)^2
+    const bool stats = first && a.stat_partial != nullptr;
+    const double pivot = stats ? a.pivot[beam] : 0.0;
+    double s1 = 0.0, s2 = 0.0;
     int pass0 = 0;  // first row of the current pass
 #pragma unroll
     for (int j = 0; j < D; ++j) {
@@ -527,6 +531,20 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
                         o[p] = xl;
                     if (p >= hi0 && p < hi1)
                         o[p + hp] = xh;
+                    if (stats) {
+                        // every output is stored by exactly one lane of one block: its statistics are
+                        // taken here, on the final value, and cost no pass over the buffer
+                        if (p >= lo0 && p < lo1) {
+                            const double dl = static_cast<double>(xl) - pivot;
+                            s1 += dl;
+                            s2 = fma(dl, dl, s2);
+                        }
+                        if (p >= hi0 && p < hi1) {
+                            const double dh = static_cast<double>(xh) - pivot;
+                            s1 += dh;
+                            s2 = fma(dh, dh, s2);
+                        }
+                    }
                 }
             } else {
 #pragma unroll
@@ -542,6 +560,32 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         pass0 = j + 1;
         if (j + 1 < D)
             __syncwarp();  // the regions are rewritten by the next pass
+    }
+    if (stats) {
+        // fixed order: lanes by shuffles, warps by index, blocks by the finishing kernel
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+            s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        }
+        double* wsum = reinterpret_cast<double*>(smem + 128) + 2 * warp;   // the hand-over state is dead by now
+        __syncwarp();
+        if (lane_pinned == 0) {
+            wsum[0] = s1;
+            wsum[1] = s2;
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(NCW * 32) : "memory");
+        if (tid == 0) {
+            double b1 = 0.0, b2 = 0.0;
+            const double* ws = reinterpret_cast<const double*>(smem + 128);
+            for (int k = 0; k < NCW; ++k) {
+                b1 += ws[2 * k];
+                b2 += ws[2 * k + 1];
+            }
+            double* dst = a.stat_partial + (static_cast<int64_t>(beam) * a.stat_stride + a.stat_off + lin2) * 2;
+            dst[0] = b1;
+            dst[1] = b2;
+        }
     }
 }
 

@@ -259,6 +259,73 @@ def test_detect_matches_oracle(oracle, dtype):
         plan.detect(out[:, :, 1:], 3.0)            # misaligned view
 
 
+def _check_detect(oracle, host_out, results, events, nsig, cap):
+    for b in range(len(results)):
+        mu, sg, thr, ev, val = oracle.detect(host_out[b], nsig)
+        r = results[b]
+        assert abs(r["mean"] - mu) <= 1e-12 * max(1.0, abs(mu)) and abs(r["sigma"] - sg) <= 1e-11 * sg
+        assert abs(r["threshold"] - thr) <= 1e-11 * abs(thr)
+        assert r["count"] == len(ev) > 0 and len(ev) <= cap
+        got = events[b]
+        order = np.lexsort((got["t"], got["dm"]))
+        assert (np.stack([got["t"][order], got["dm"][order]], axis=1) == ev).all()
+        assert (got["value"][order] == val.astype(np.float32)).all()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "u8"])
+def test_execute_detect_fused(oracle, dtype):
+    """dedisp_execute_detect / dedisp_execute_detect_host (PAPER.md:76 fused behind the hot path): the
+    register-window kernel accumulates the statistics in its flush.  The de-dispersed buffer is checked
+    against the brute-force oracle, then mean / sigma / threshold (1e-11) and the event SET against
+    oracle.detect on that buffer; the host entry (several time pieces, events only) returns the same
+    set; a subband plan takes the unfused route with the same definition."""
+    cf = synth.scaled(synth.configs()[1], dtype=dtype, ndm=37, n_out=2 * 32768 + 1000 + 3)     # cfg-1 band and DM grid
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    assert plan.resolved_kernel(dd.U8 if dtype == "u8" else dd.F32) == dd.KERNEL_WINDOW and plan.window_info()["nband"] == 1
+    nsig, cap = 3.5, 1 << 16
+    out, results, events = plan.execute_detect(to_dev(x), cf.n_out, nsig, capacity=cap)
+    assert plan.last_launches == 1 + 2 + 2           # pivot, pairify + one band, finish + threshold scan
+    host = out.cpu().numpy()
+    for b in range(2):
+        if dtype == "u8":
+            assert (host[b] == oracle.brute_u8(x[b], tab, cf.n_out)).all()
+        else:
+            ref, sa = oracle.brute_f32(x[b], tab, cf.n_out)
+            check_f32(host[b], ref, sa)
+    _check_detect(oracle, host, results, events, nsig, cap)
+    # the two-pass detection on the same buffer: same statistics (another summation order), same events
+    r2, e2 = plan.detect(out, nsig, capacity=cap)
+    for b in range(2):
+        assert abs(r2[b]["sigma"] - results[b]["sigma"]) <= 1e-11 * r2[b]["sigma"] and r2[b]["count"] == results[b]["count"]
+    # events-only host entry: pieces of 32768 outputs, nothing but triplets and statistics come back
+    rh, eh = plan.execute_detect_host(x, cf.n_out, nsig, capacity=cap)
+    if dtype == "u8":
+        _check_detect(oracle, host, rh, eh, nsig, cap)
+    else:
+        # The host entry de-disperses in time pieces: tiles, and with them the places where partial sums are
+        # handed over, fall elsewhere, so its (device-resident) fp32 buffer may differ from `host` in the
+        # last bit of some samples (reading R13).  Statistics agree to fp32 rounding; events may differ
+        # only within that rounding of the threshold.
+        for b in range(2):
+            mu, sg, thr, ev, val = oracle.detect(host[b], nsig)
+            assert abs(rh[b]["mean"] - mu) <= 1e-7 * sg and abs(rh[b]["sigma"] - sg) <= 1e-7 * sg
+            a = set(zip(eh[b]["t"].tolist(), eh[b]["dm"].tolist()))
+            c = set(map(tuple, ev.tolist()))
+            for (t, d) in a ^ c:
+                assert abs(host[b][d, t] - thr) <= 1e-5 * np.abs(x[b]).sum(axis=0).max()
+    plan.close()
+    # unfused route (subband plan), same definition
+    cs = small_cfg(dtype, nchans=128, ndm=96, n_out=2048 + 33, step=0.25, nsub=8, nfine=12)
+    full = oracle.shift_table(cs.nchans, cs.f_top_mhz, cs.df_mhz, cs.t_samp_ms, cs.dm_list)
+    xs = synth.make_input(cs, cs.n_out + int(full.max()), [(18, 500, 30, 1.5)], {18: full[18]})[None]
+    ps = dd.Plan(**cs.plan_args())
+    outs, rs, es = ps.execute_detect(to_dev(xs[:, :, :cs.n_out + ps.max_delay].copy()), cs.n_out, 3.0, capacity=cap)
+    _check_detect(oracle, outs.cpu().numpy(), rs, es, 3.0, cap)
+    rsh, esh = ps.execute_detect_host(np.ascontiguousarray(xs[:, :, :cs.n_out + ps.max_delay]), cs.n_out, 3.0, capacity=cap)
+    _check_detect(oracle, outs.cpu().numpy(), rsh, esh, 3.0, cap)      # one piece, same kernels: same buffer
+
+
 def test_kernel_timing_hook(oracle):
     cf = small_cfg()
     tab, x = make_case(oracle, cf)
