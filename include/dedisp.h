@@ -332,6 +332,44 @@ DEDISP_API dedisp_status dedisp_bin(const void *in, void *out, int64_t nrows, in
                                     int64_t out_stride, int nb, void *cuda_stream);
 
 /*
+ * Multi-pass subband survey ("each pass will bin the data using a different binning
+ * factor ... For each pass the DM range is partitioned, each range being dSub_DM apart"; the three
+ * stages of PAPER.md:137-143; Tables 1 and 4).  Pass i covers the trials dm_low + d*dm_step,
+ * d = 0 .. ndm-1 (one multiply and one add in fp64), in groups of nfine = dSub_DM / dDM trials around a
+ * nominal DM, on the input binned by `bin`.  Per pass, on the device and without a round trip to the
+ * host: (i) dedisp_bin by `bin` (skipped for bin 1), (ii) subband stage 1 and
+ * (iii) stage 2 of a subband plan created with t_samp * bin (dedisp_plan_create with nsub, nfine).
+ *
+ * A survey over nsamp input samples per channel needs nsamp + dedisp_survey_max_delay samples
+ * (= max over passes of bin * max_delay of the pass's plan, in unbinned samples; R17) and
+ * yields nsamp / bin outputs per trial of a pass (eq. 8).
+ *
+ *   in     DEVICE float [nbeams][nchans][in_stride], in_stride >= nsamp + max_delay, a multiple of 4,
+ *          16-byte aligned
+ *   out    DEVICE float, dedisp_survey_out_layout's `total` elements: pass i is the dense block
+ *          [nbeams][ndm_i][stride_i] at element offset_i, nout_i = nsamp / bin_i valid samples per row
+ * dedisp_survey_reserve (blocking) sizes the plans' scratch and the binned buffer; dedisp_survey_execute
+ * is asynchronous on cuda_stream and returns DEDISP_ESTATE without a covering reserve.  fp32 input only.
+ * One execute per survey in flight.  dedisp_survey_pass_plan lends pass i's plan for the table getters
+ * (do not destroy it).
+ */
+typedef struct dedisp_survey dedisp_survey; /* opaque, library-owned */
+typedef struct { double dm_low, dm_step; int ndm, nfine, bin; } dedisp_pass;
+DEDISP_API dedisp_status dedisp_survey_create(dedisp_survey **survey, int nchans, double f_top_mhz, double df_mhz,
+                                              double t_samp_ms, int nsub, const dedisp_pass *passes, int npass);
+DEDISP_API dedisp_status dedisp_survey_destroy(dedisp_survey *survey);
+DEDISP_API int dedisp_survey_npass(const dedisp_survey *survey);
+DEDISP_API int64_t dedisp_survey_max_delay(const dedisp_survey *survey);
+DEDISP_API const dedisp_plan *dedisp_survey_pass_plan(const dedisp_survey *survey, int pass);
+/* HOST arrays of npass int64 (any may be NULL) and the total element count of `out`. */
+DEDISP_API dedisp_status dedisp_survey_out_layout(const dedisp_survey *survey, int64_t nsamp, int nbeams, int64_t *offset,
+                                                  int64_t *stride, int64_t *nout, int64_t *total);
+DEDISP_API dedisp_status dedisp_survey_reserve(dedisp_survey *survey, int64_t nsamp, int nbeams);
+DEDISP_API dedisp_status dedisp_survey_execute(dedisp_survey *survey, const void *in, void *out, int64_t nsamp,
+                                               int64_t in_stride, int nbeams, void *cuda_stream);
+DEDISP_API int dedisp_survey_last_launches(const dedisp_survey *survey);
+
+/*
  * Register-only FP32 add microbenchmark: the measured denominator of the brute-force roofline.  The
  * method is nchans adds per output sample ("N_c additions"), so its ceiling is the
  * rate at which the SMs add when no operand comes from memory (nominally

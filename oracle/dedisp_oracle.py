@@ -266,3 +266,36 @@ def bin_samples(x, nb):
     for i in range(1, nb):
         acc = (acc + v[..., i]).astype(np.float32)
     return (acc / np.float32(nb)).astype(np.float32), v.astype(np.float64).mean(axis=-1)
+
+
+def survey(x, nchans, f_top_mhz, df_mhz, t_samp_ms, nsub, passes, nsamp, want_sumabs=True):
+    """Multi-pass subband survey (PAPER.md:58-60 survey plan; :137-155 the three stages; Tables 1 / 4):
+    for every pass (dm_low, dm_step, ndm, nfine, bin), in the paper's order,
+      (i)   binning: xb = bin_samples(x, bin)            (fp32-defined, reading R16; bin = 1: x itself)
+      (ii)  subband stage 1 and (iii) stage 2: subband(xb, tables for t_samp * bin and the pass's DM list
+            dm_low + d * dm_step, nsub, nfine), n_i = nsamp // bin outputs per trial (eq. 8: n_samp / b_i).
+    Reading R17: a survey over nsamp input samples needs nsamp + M samples per channel,
+    M = max_i bin_i * max_delay_i (unbinned samples); `survey_max_delay` returns it.
+    Returns [(out_i, sumabs_i, dm_list_i)].  No arithmetic of its own beyond the DM list: every step is a
+    pinned oracle function.  Pins (tests/test_oracle_pins.py): one pass with bin 1 is `subband`; Table 4
+    gives 3102 trials and 136 nominal DMs; a noise-free pulse is recovered at its trial in its pass."""
+    res = []
+    for (dm_low, dm_step, ndm, nfine, b) in passes:
+        dm = float(dm_low) + np.arange(int(ndm), dtype=np.float64) * float(dm_step)
+        tab = subband_tables(nchans, f_top_mhz, df_mhz, t_samp_ms * b, dm, nsub, int(nfine))
+        xb = np.ascontiguousarray(x if b == 1 else bin_samples(x, b)[0])
+        n_i = int(nsamp) // b
+        if n_i + tab.max_delay > xb.shape[1]:
+            raise ValueError("survey: input too short for pass with bin %d" % b)
+        r = subband(xb, tab, n_i, want_sumabs=want_sumabs)
+        res.append((r[0], r[1], dm) if want_sumabs else (r, None, dm))
+    return res
+
+
+def survey_max_delay(nchans, f_top_mhz, df_mhz, t_samp_ms, nsub, passes):
+    """Unbinned input samples a survey needs beyond nsamp: max over passes of bin * max_delay(pass)."""
+    m = 0
+    for (dm_low, dm_step, ndm, nfine, b) in passes:
+        dm = float(dm_low) + np.arange(int(ndm), dtype=np.float64) * float(dm_step)
+        m = max(m, b * subband_tables(nchans, f_top_mhz, df_mhz, t_samp_ms * b, dm, nsub, int(nfine)).max_delay)
+    return int(m)

@@ -50,6 +50,15 @@ _SIGS = {
     "dedisp_execute_detect_host": (_int, [_vp, _vp, _int, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
     "dedisp_bin": (_int, [_vp, _vp, _i64, _i64, _i64, _i64, _int, _vp]),
+    "dedisp_survey_create": (_int, [_c.POINTER(_vp), _int, _dbl, _dbl, _dbl, _int, _vp, _int]),
+    "dedisp_survey_destroy": (_int, [_vp]),
+    "dedisp_survey_npass": (_int, [_vp]),
+    "dedisp_survey_max_delay": (_i64, [_vp]),
+    "dedisp_survey_pass_plan": (_vp, [_vp, _int]),
+    "dedisp_survey_out_layout": (_int, [_vp, _i64, _int, _vp, _vp, _vp, _vp]),
+    "dedisp_survey_reserve": (_int, [_vp, _i64, _int]),
+    "dedisp_survey_execute": (_int, [_vp, _vp, _vp, _i64, _i64, _int, _vp]),
+    "dedisp_survey_last_launches": (_int, [_vp]),
     "dedisp_fadd_microbench": (_int, [_int, _int, _int, _vp, _vp, _vp, _vp]),
     "dedisp_strerror": (_c.c_char_p, [_int]),
     "dedisp_version": (_c.c_char_p, []),
@@ -393,6 +402,84 @@ class Stream:
     def close(self):
         if getattr(self, "_h", None):
             _check(lib().dedisp_stream_destroy(self._h), "dedisp_stream_destroy")
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class _Pass(ctypes.Structure):
+    _fields_ = [("dm_low", _dbl), ("dm_step", _dbl), ("ndm", _int), ("nfine", _int), ("bin", _int)]
+
+
+class Survey:
+    """dedisp_survey_*: passes = [(dm_low, dm_step, ndm, nfine, bin), ...] (Tables 1 / 4)."""
+
+    def __init__(self, nchans, f_top_mhz, df_mhz, t_samp_ms, nsub, passes):
+        arr = (_Pass * len(passes))(*[_Pass(float(a), float(b), int(c), int(d), int(e)) for (a, b, c, d, e) in passes])
+        h = _vp()
+        _check(lib().dedisp_survey_create(ctypes.byref(h), int(nchans), float(f_top_mhz), float(df_mhz), float(t_samp_ms),
+                                          int(nsub), ctypes.addressof(arr), len(passes)), "dedisp_survey_create")
+        self._h, self.nchans, self.nsub, self.passes = h, int(nchans), int(nsub), [tuple(p) for p in passes]
+        self._reserved = (-1, 0)
+
+    @property
+    def max_delay(self):
+        return int(lib().dedisp_survey_max_delay(self._h))
+
+    @property
+    def last_launches(self):
+        return int(lib().dedisp_survey_last_launches(self._h))
+
+    def pass_tables(self, i):
+        """(s1, s2, nominal_dm, maxshift2, max_delay) of pass i's subband plan."""
+        ph = lib().dedisp_survey_pass_plan(self._h, int(i))
+        ndm, nfine = self.passes[i][2], self.passes[i][3]
+        nco = ndm // nfine
+        s1 = np.empty((nco, self.nchans), dtype=np.int32)
+        s2 = np.empty((ndm, self.nsub), dtype=np.int32)
+        nom = np.empty(nco, dtype=np.float64)
+        m2 = np.empty(nco, dtype=np.int32)
+        _check(lib().dedisp_plan_get_subband_shifts(ph, s1.ctypes.data, s2.ctypes.data, nom.ctypes.data, m2.ctypes.data),
+               "dedisp_plan_get_subband_shifts")
+        return s1, s2, nom, m2, int(lib().dedisp_plan_max_delay(ph))
+
+    def out_layout(self, nsamp, nbeams=1):
+        n = len(self.passes)
+        off, st, no = (np.zeros(n, dtype=np.int64) for _ in range(3))
+        tot = _i64(0)
+        _check(lib().dedisp_survey_out_layout(self._h, int(nsamp), int(nbeams), off.ctypes.data, st.ctypes.data,
+                                              no.ctypes.data, ctypes.addressof(tot)), "dedisp_survey_out_layout")
+        return off, st, no, int(tot.value)
+
+    def execute(self, x, nsamp, stream=None):
+        """x: CUDA float32 [(nbeams,) nchans, >= nsamp + max_delay].  Returns one tensor view
+        [(nbeams,) ndm_i, nsamp // bin_i] per pass (all inside one output buffer)."""
+        import torch
+        x3 = x if x.dim() == 3 else x.unsqueeze(0)
+        if not x.is_cuda or x.dtype != torch.float32 or x3.shape[1] != self.nchans or x3.stride(2) != 1 or \
+                (x3.shape[0] > 1 and x3.stride(0) != x3.shape[1] * x3.stride(1)):
+            raise DedispError(ESHAPE, "dedisp_survey_execute")
+        nb = x3.shape[0]
+        if nsamp > self._reserved[0] or nb > self._reserved[1]:
+            _check(lib().dedisp_survey_reserve(self._h, int(nsamp), int(nb)), "dedisp_survey_reserve")
+            self._reserved = (max(self._reserved[0], int(nsamp)), max(self._reserved[1], int(nb)))
+        off, st, no, tot = self.out_layout(nsamp, nb)
+        out = torch.empty(max(tot, 4), dtype=torch.float32, device=x.device)
+        _check(lib().dedisp_survey_execute(self._h, x3.data_ptr(), out.data_ptr(), int(nsamp), int(x3.stride(1)), int(nb),
+                                           _stream_ptr(stream)), "dedisp_survey_execute")
+        views = []
+        for i, p in enumerate(self.passes):
+            v = out[off[i]:off[i] + nb * p[2] * st[i]].view(nb, p[2], int(st[i]))[:, :, :int(no[i])]
+            views.append(v if x.dim() == 3 else v[0])
+        return views
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _check(lib().dedisp_survey_destroy(self._h), "dedisp_survey_destroy")
             self._h = None
 
     def __del__(self):

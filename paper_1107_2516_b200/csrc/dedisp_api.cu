@@ -120,6 +120,16 @@ struct dedisp_stream {
 
 extern "C" int64_t dedisp_plan_scratch_bytes(const dedisp_plan* p, int64_t nsamp_out, int nbeams);
 
+struct dedisp_survey {
+    int nchans = 0, nsub = 0;
+    double f_top = 0, df = 0, t_samp = 0;
+    std::vector<dedisp_pass> passes;
+    std::vector<dedisp_plan*> plans;  // one subband plan per pass, created with t_samp * bin
+    int64_t max_delay = 0;            // unbinned input samples beyond nsamp: max_i bin_i * max_delay_i
+    DevBuf binned;                    // [nbeams][nchans][stride] of the pass being executed (bin > 1)
+    int last_launches = 0;
+};
+
 namespace {
 
 size_t in_size(dedisp_dtype t) { return t == DEDISP_F32 ? 4 : 1; }
@@ -1222,6 +1232,156 @@ dedisp_status dedisp_bin(const void* in, void* out, int64_t nrows, int64_t nsamp
     if (in_stride < nsamp || out_stride < nsamp / nb)
         return DEDISP_ESHAPE;
     return launch_bin(in, out, nrows, nsamp / nb, in_stride, out_stride, nb, cuda_stream) == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
+
+// ---- multi-pass subband survey (Tables 1 and 4) ---------------------------
+
+dedisp_status dedisp_survey_create(dedisp_survey** survey, int nchans, double f_top_mhz, double df_mhz, double t_samp_ms,
+                                   int nsub, const dedisp_pass* passes, int npass)
+{
+    if (!survey)
+        return DEDISP_EINVAL;
+    *survey = nullptr;
+    if (!passes || npass <= 0 || nsub <= 0)
+        return DEDISP_EINVAL;
+    dedisp_survey* s = new (std::nothrow) dedisp_survey;
+    if (!s)
+        return DEDISP_ENOMEM;
+    s->nchans = nchans;
+    s->nsub = nsub;
+    s->f_top = f_top_mhz;
+    s->df = df_mhz;
+    s->t_samp = t_samp_ms;
+    dedisp_status st = DEDISP_OK;
+    try {
+        for (int i = 0; i < npass && st == DEDISP_OK; ++i) {
+            const dedisp_pass& p = passes[i];
+            if (p.ndm <= 0 || p.nfine <= 0 || p.bin <= 0 || !(p.dm_step >= 0.0) || !(p.dm_low >= 0.0)) {
+                st = DEDISP_EINVAL;
+                break;
+            }
+            std::vector<double> dm(p.ndm);
+            for (int d = 0; d < p.ndm; ++d)
+                dm[d] = p.dm_low + static_cast<double>(d) * p.dm_step;  // one multiply, one add, each rounded
+            dedisp_plan* plan = nullptr;
+            st = dedisp_plan_create(&plan, nchans, f_top_mhz, df_mhz, t_samp_ms * p.bin, dm.data(), p.ndm, nsub, p.nfine);
+            if (st == DEDISP_OK) {
+                s->passes.push_back(p);
+                s->plans.push_back(plan);
+                s->max_delay = std::max(s->max_delay, plan->max_delay * p.bin);
+            }
+        }
+    } catch (const std::bad_alloc&) {
+        st = DEDISP_ENOMEM;
+    }
+    if (st != DEDISP_OK) {
+        dedisp_survey_destroy(s);
+        return st;
+    }
+    *survey = s;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_survey_destroy(dedisp_survey* s)
+{
+    if (!s)
+        return DEDISP_OK;
+    for (dedisp_plan* p : s->plans)
+        dedisp_plan_destroy(p);
+    s->binned.release();
+    delete s;
+    return DEDISP_OK;
+}
+
+int dedisp_survey_npass(const dedisp_survey* s) { return s ? static_cast<int>(s->plans.size()) : -1; }
+int64_t dedisp_survey_max_delay(const dedisp_survey* s) { return s ? s->max_delay : -1; }
+int dedisp_survey_last_launches(const dedisp_survey* s) { return s ? s->last_launches : -1; }
+
+const dedisp_plan* dedisp_survey_pass_plan(const dedisp_survey* s, int pass)
+{
+    return s && pass >= 0 && pass < static_cast<int>(s->plans.size()) ? s->plans[pass] : nullptr;
+}
+
+dedisp_status dedisp_survey_out_layout(const dedisp_survey* s, int64_t nsamp, int nbeams, int64_t* offset,
+                                       int64_t* stride, int64_t* nout, int64_t* total)
+{
+    if (!s || nsamp < 0 || nbeams <= 0)
+        return DEDISP_EINVAL;
+    int64_t off = 0;
+    for (size_t i = 0; i < s->plans.size(); ++i) {
+        const int64_t n = nsamp / s->passes[i].bin, st = round_up(n, 4);
+        if (offset)
+            offset[i] = off;
+        if (stride)
+            stride[i] = st;
+        if (nout)
+            nout[i] = n;
+        off += static_cast<int64_t>(nbeams) * s->plans[i]->ndm * st;
+    }
+    if (total)
+        *total = off;
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_survey_reserve(dedisp_survey* s, int64_t nsamp, int nbeams)
+{
+    if (!s || nsamp < 0 || nbeams <= 0)
+        return DEDISP_EINVAL;
+    size_t need = 0;
+    for (size_t i = 0; i < s->plans.size(); ++i) {
+        const int b = s->passes[i].bin;
+        const dedisp_status st = reserve(s->plans[i], DEDISP_F32, nsamp / b, nbeams);
+        if (st != DEDISP_OK)
+            return st;
+        if (b > 1)
+            need = std::max(need, static_cast<size_t>(nbeams) * s->nchans * round_up((nsamp + s->max_delay) / b, 16) * 4);
+    }
+    if (s->binned.ensure(need) != cudaSuccess) {
+        cudaGetLastError();
+        return DEDISP_ENOMEM;
+    }
+    return DEDISP_OK;
+}
+
+dedisp_status dedisp_survey_execute(dedisp_survey* s, const void* in, void* out, int64_t nsamp, int64_t in_stride,
+                                    int nbeams, void* cuda_stream)
+{
+    if (!s || !in || !out || nsamp < 0 || nbeams <= 0)
+        return DEDISP_EINVAL;
+    if (in_stride < nsamp + s->max_delay || in_stride % 4 != 0 || (reinterpret_cast<uintptr_t>(in) & 15) != 0 ||
+        (reinterpret_cast<uintptr_t>(out) & 15) != 0)
+        return DEDISP_ESHAPE;
+    s->last_launches = 0;
+    int64_t off = 0;
+    float* o = static_cast<float*>(out);
+    for (size_t i = 0; i < s->plans.size(); ++i) {
+        dedisp_plan* plan = s->plans[i];
+        const int b = s->passes[i].bin;
+        const int64_t n = nsamp / b, ostride = round_up(n, 4);
+        const void* src = in;
+        int64_t sstride = in_stride;
+        if (b > 1) {
+            // stage (i), on the device: every row of nsamp + max_delay samples -> (nsamp + max_delay) / b
+            const int64_t lb = (nsamp + s->max_delay) / b;
+            sstride = round_up(lb, 16);
+            if (static_cast<size_t>(nbeams) * s->nchans * sstride * 4 > s->binned.bytes)
+                return DEDISP_ESTATE;  // dedisp_survey_reserve was not called for this shape
+            if (launch_bin(in, s->binned.p, static_cast<int64_t>(nbeams) * s->nchans, lb, in_stride, sstride, b,
+                           cuda_stream) != 0)
+                return DEDISP_ECUDA;
+            ++s->last_launches;
+            src = s->binned.p;
+        }
+        // stages (ii) and (iii): the pass's subband plan (tables for t_samp * b)
+        if (n > 0) {
+            const dedisp_status st = execute_device(plan, src, o + off, DEDISP_F32, n, sstride, ostride, nbeams, cuda_stream);
+            if (st != DEDISP_OK)
+                return st;
+            s->last_launches += plan->last_launches;
+        }
+        off += static_cast<int64_t>(nbeams) * plan->ndm * ostride;
+    }
+    return DEDISP_OK;
 }
 
 dedisp_status dedisp_fadd_microbench(int packed, int iters, int repeats, float* ms, double* adds, int* nsm_out,

@@ -126,3 +126,27 @@ def test_max_chunk_follows_eq3():
     used = lambda n: 4 * (2 * cf.nchans * (M + 16 + n) * 1 + cf.ndm * n * 4)
     assert n > 0 and n % 16 == 0 and used(n) <= mem < used(n + 32)
     assert p.max_chunk(dd.U8, 1 << 20, nbeams=4) == 0
+
+
+def test_survey_tables_match_oracle_table4(oracle):
+    """dedisp_survey_create on the paper's Table 4 plan (1024 channels, 16 MHz at 300 MHz; 3102 trials in
+    3 passes with bin 1 / 2 / 4 and 22 / 24 / 24 fine trials per nominal DM): every pass's subband tables,
+    built for t_samp * bin, equal the oracle's; the survey's input overlap is max_i bin_i * max_delay_i."""
+    from test_oracle_pins import table4_passes
+    nch, ft, df, ts, nsub = 1024, 308.0, 16.0 / 1024, 0.1, 32
+    passes = table4_passes()
+    sv = dd.Survey(nch, ft, df, ts, nsub, passes)
+    assert sv.max_delay == oracle.survey_max_delay(nch, ft, df, ts, nsub, passes)
+    for i, (lo, step, ndm, nfine, b) in enumerate(passes):
+        dm = lo + np.arange(ndm, dtype=np.float64) * step
+        t = oracle.subband_tables(nch, ft, df, ts * b, dm, nsub, nfine)
+        s1, s2, nom, m2, md = sv.pass_tables(i)
+        assert (s1 == t.s1).all() and (s2 == t.s2).all() and (nom == t.nominal).all() and (m2 == t.maxshift2).all()
+        assert md == t.max_delay
+    off, st, no, tot = sv.out_layout(8192, 2)
+    assert list(no) == [8192, 4096, 2048] and off[0] == 0 and off[1] == 2 * 1782 * 8192
+    assert tot == 2 * (1782 * 8192 + 696 * 4096 + 624 * 2048)
+    sv.close()
+    for bad in ([(0.0, 0.1, 10, 3, 1)], [(0.0, 0.1, 12, 3, 0)], [(-1.0, 0.1, 12, 3, 1)], []):
+        with pytest.raises(dd.DedispError):
+            dd.Survey(64, 150.0, 0.1, 0.1, 8, bad)

@@ -689,3 +689,81 @@ def test_binning_matches_oracle_and_feeds_a_pass(oracle):
     got = plan.execute(dd.bin_samples(to_dev(raw), 2), cfb.n_out).cpu().numpy()
     ref, sa = oracle.brute_f32(oracle.bin_samples(raw, 2)[0], tab, cfb.n_out)
     check_f32(got, ref, sa)
+
+
+def test_survey_table4_matches_oracle_chain(oracle):
+    """dedisp_survey_execute on the paper's Table 4 plan: 1024 channels over 16 MHz at
+    300 MHz, 3 passes (bin 1 / 2 / 4; 22 / 24 / 24 fine trials per nominal DM, i.e. row tiles that are no
+    multiple of the long-tile kernel's 16 rows), 3102 trials, 8192 input samples.  Per pass binning ->
+    stage 1 -> stage 2 run on the device; every output against oracle.survey (bin_samples -> subband)."""
+    from test_oracle_pins import table4_passes
+    nch, ft, df, ts, nsub, nsamp = 1024, 308.0, 16.0 / 1024, 0.1, 32, 8192
+    passes = table4_passes()
+    sv = dd.Survey(nch, ft, df, ts, nsub, passes)
+    M = sv.max_delay
+    cf = synth.Config("table4", nch, ft, df, ts, nsamp, 1, 0.0, seed=404)
+    x = synth.make_input(cf, nsamp + M)
+    # a pulse at a nominal trial of pass 3 (unbinned dispersion curve), 12.8 ms wide
+    dmp = passes[2][0] + (24 + 12) * passes[2][1]
+    row = oracle.shift_table(nch, ft, df, ts, np.array([dmp]))[0]
+    for c in range(nch):
+        x[c, 1000 + row[c]:1000 + row[c] + 128] += 1.0
+    outs = sv.execute(to_dev(x), nsamp)
+    assert sv.last_launches == 2 * 3 + 2                     # two stages per pass, binning for bin 2 and 4
+    ref = oracle.survey(x, nch, ft, df, ts, nsub, passes, nsamp)
+    for i, (o, (r, sa, dm)) in enumerate(zip(outs, ref)):
+        assert tuple(o.shape) == r.shape == (passes[i][2], nsamp // passes[i][4])
+        check_f32(o.cpu().numpy(), r, sa)
+    box = outs[2].cpu().numpy()[:, 1000 // 4:(1000 + 128) // 4].sum(axis=1)
+    assert int(np.argmax(box)) == 24 + 12
+    sv.close()
+
+
+def test_survey_small_two_beams(oracle):
+    nch, ft, df, ts, nsub, nsamp = 64, 150.0, 0.1, 0.2, 8, 4096 + 40
+    passes = [(0.0, 0.25, 24, 12, 1), (6.0, 0.5, 12, 6, 2), (12.0, 1.0, 9, 3, 3)]
+    sv = dd.Survey(nch, ft, df, ts, nsub, passes)
+    M = sv.max_delay
+    rng = np.random.default_rng(9)
+    x = rng.standard_normal((2, nch, nsamp + M)).astype(np.float32)
+    outs = sv.execute(to_dev(x), nsamp)
+    for b in range(2):
+        ref = oracle.survey(x[b], nch, ft, df, ts, nsub, passes, nsamp)
+        for o, (r, sa, dm) in zip(outs, ref):
+            check_f32(o[b].cpu().numpy(), r, sa)
+    with pytest.raises(dd.DedispError):
+        sv.execute(to_dev(x[:, :, :nsamp + M - 1]), nsamp)        # one input sample short
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_dm_sharded_execute_equals_the_whole(oracle, world):
+    """"The DM range is split among these threads, such that each will process the same input
+    buffer for different DM values."  Every rank's plan is built from its shard.dm_slice of the DM list
+    (subband plans: whole coarse groups) and executed on the SAME input; the concatenation of the shards'
+    rows is the whole result: against the oracle's one-plan result, brute force (uint8, bit-exact) and
+    two-stage (fp32).  The ranks run one after the other on the one GPU: the path has no exchange step."""
+    from paper_1107_2516_b200 import shard
+    # brute force: cfg-1 band, 67 trials (no multiple of the world size), uint8
+    cf = synth.scaled(synth.configs()[1], dtype="u8", ndm=67, n_out=4096 + 100)
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
+    x = synth.make_input(cf, cf.n_out + int(tab.max()))          # the extent of the WHOLE list, on every rank
+    xd = to_dev(x)
+    parts = []
+    for rank in range(world):
+        lo, hi = shard.dm_slice(cf.ndm, world, rank)
+        plan = dd.Plan(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list[lo:hi])
+        assert (plan.shifts() == tab[lo:hi]).all() and plan.max_delay <= int(tab.max())
+        parts.append(plan.execute(xd, cf.n_out).cpu().numpy())
+    assert (np.concatenate(parts, axis=0) == oracle.brute_u8(x, tab, cf.n_out)).all()
+    # two-stage: cfg-4 band, 256 channels in 4 subbands, 5 coarse groups of 32 trials
+    cs = synth.scaled(synth.configs()[4], nchans=256, nsub=4, ndm=5 * 32, n_out=4096 + 24)
+    t = oracle.subband_tables(cs.nchans, cs.f_top_mhz, cs.df_mhz, cs.t_samp_ms, cs.dm_list, cs.nsub, cs.nfine)
+    xs = synth.make_input(cs, cs.n_out + t.max_delay)
+    xsd = to_dev(xs)
+    parts = []
+    for rank in range(world):
+        lo, hi = shard.dm_slice(cs.ndm, world, rank, multiple=cs.nfine)
+        plan = dd.Plan(cs.nchans, cs.f_top_mhz, cs.df_mhz, cs.t_samp_ms, cs.dm_list[lo:hi], cs.nsub, cs.nfine)
+        parts.append(plan.execute(xsd, cs.n_out).cpu().numpy())
+    ref, sa = oracle.subband(xs, t, cs.n_out)
+    check_f32(np.concatenate(parts, axis=0), ref, sa)

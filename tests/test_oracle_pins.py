@@ -468,3 +468,72 @@ def test_bin_samples_pins(oracle):
         b32, b64 = oracle.bin_samples(g, nb)
         assert b32.shape == (5, 999 // nb)
         assert np.abs(b32 - b64).max() <= nb * np.spacing(np.float32(np.abs(g).max()))
+
+
+def table4_passes():
+    """(dm_low, dm_step, ndm, nfine, bin) per pass from tests/golden/table4_plan.txt (Table 4)."""
+    out = []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "table4_plan.txt")):
+        f = line.split("#")[0].split()
+        if f:
+            lo, hi, ddm, b, dsub = float(f[1]), float(f[2]), float(f[3]), int(f[4]), float(f[5])
+            out.append((lo, ddm, int(round((hi - lo) / ddm)), int(round(dsub / ddm)), b))
+    return out
+
+
+def test_survey_plan_table4_counts():
+    """PAPER.md Table 1 / 4 -> 3102 trials, 136 nominal DMs, 22 / 24 / 24 fine trials per nominal DM
+    (SURVEY.md A12), passes contiguous in DM."""
+    ps = table4_passes()
+    assert [p[2] for p in ps] == [1782, 696, 624] and sum(p[2] for p in ps) == 3102
+    assert [p[3] for p in ps] == [22, 24, 24] and [p[4] for p in ps] == [1, 2, 4]
+    assert [p[2] // p[3] for p in ps] == [81, 29, 26] and sum(p[2] // p[3] for p in ps) == 136
+    for a, b in zip(ps, ps[1:]):
+        assert abs(a[0] + a[2] * a[1] - b[0]) < 1e-9
+
+
+def test_survey_single_pass_is_subband_and_binning_chain(oracle):
+    """oracle.survey: one pass with bin 1 IS oracle.subband on that DM list; a pass with bin 2 is
+    bin_samples followed by subband with 2 * t_samp (stages (i)-(iii))."""
+    nch, ft, df, ts, nsub = 64, 150.0, 0.1, 0.2, 8
+    rng = np.random.default_rng(44)
+    passes = [(0.0, 0.25, 24, 12, 1), (6.0, 0.5, 12, 6, 2)]
+    nsamp = 1000
+    M = oracle.survey_max_delay(nch, ft, df, ts, nsub, passes)
+    x = rng.standard_normal((nch, nsamp + M)).astype(np.float32)
+    res = oracle.survey(x, nch, ft, df, ts, nsub, passes, nsamp)
+    dm0 = 0.0 + np.arange(24) * 0.25
+    t0 = oracle.subband_tables(nch, ft, df, ts, dm0, nsub, 12)
+    ref0, sa0 = oracle.subband(x, t0, nsamp)
+    assert (res[0][0] == ref0).all() and (res[0][1] == sa0).all() and (res[0][2] == dm0).all()
+    xb = oracle.bin_samples(x, 2)[0]
+    dm1 = 6.0 + np.arange(12) * 0.5
+    t1 = oracle.subband_tables(nch, ft, df, 2 * ts, dm1, nsub, 6)
+    ref1, _ = oracle.subband(np.ascontiguousarray(xb), t1, nsamp // 2)
+    assert res[1][0].shape == (12, nsamp // 2) and (res[1][0] == ref1).all()
+    assert M == max(t0.max_delay, 2 * t1.max_delay)
+
+
+def test_survey_recovers_a_pulse_in_each_pass(oracle):
+    """A noise-free boxcar pulse injected along the (unbinned) dispersion curve of a trial of each pass is
+    recovered by oracle.survey at that trial of that pass (P7 through binning and both subband stages);
+    pulses are wider than the binning and the subband smear."""
+    nch, ft, df, ts, nsub = 128, 308.0, 16.0 / 128, 0.5, 8
+    passes = [(0.0, 0.3, 44, 22, 1), (13.2, 0.5, 48, 24, 2), (37.2, 1.0, 48, 24, 4)]
+    nsamp = 4096
+    M = oracle.survey_max_delay(nch, ft, df, ts, nsub, passes)
+    x = np.zeros((nch, nsamp + M), dtype=np.float32)
+    truth = []
+    for i, (lo, step, ndm, nfine, b) in enumerate(passes):
+        d = nfine + nfine // 2                       # a nominal trial (second group) of the pass
+        dm = lo + d * step
+        row = oracle.shift_table(nch, ft, df, ts, np.array([dm]))[0]     # unbinned delays at that DM
+        t0, w = 400 + 1000 * i, 64
+        for c in range(nch):
+            x[c, t0 + row[c]:t0 + row[c] + w] += 1.0
+        truth.append((d, t0, w, b))
+    res = oracle.survey(x, nch, ft, df, ts, nsub, passes, nsamp, want_sumabs=False)
+    for (out, _, dm), (d, t0, w, b) in zip(res, truth):
+        box = out[:, t0 // b:(t0 + w) // b].sum(axis=1)
+        assert int(np.argmax(box)) == d
+        assert box[d] > 0.9 * nch * w / b            # binning averages: nch * (w / b) samples of height 1
