@@ -30,6 +30,18 @@ def test_library_exports_every_declared_symbol():
     assert "sm_100a" in dd.version()
 
 
+def test_header_compiles_as_c_and_a_c_caller_works(tmp_path):
+    """tests/abi_smoke.c: gcc -std=c99 against include/dedisp.h and the .so, run without a device."""
+    import subprocess
+    exe = str(tmp_path / "abi_smoke")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-I" + os.path.join(ROOT, "include"),
+                           os.path.join(ROOT, "tests", "abi_smoke.c"), "-o", exe, dd.LIB_PATH,
+                           "-Wl,-rpath," + os.path.dirname(dd.LIB_PATH)])
+    out = subprocess.run([exe], capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0, out.stderr
+    assert "abi_smoke ok" in out.stdout and "sm_100a" in out.stdout
+
+
 def _plan(cf, **kw):
     a = cf.plan_args()
     a.update(kw)

@@ -767,3 +767,35 @@ def test_dm_sharded_execute_equals_the_whole(oracle, world):
         parts.append(plan.execute(xsd, cs.n_out).cpu().numpy())
     ref, sa = oracle.subband(xs, t, cs.n_out)
     check_f32(np.concatenate(parts, axis=0), ref, sa)
+
+
+def test_execute_is_asynchronous_and_allocation_free(oracle):
+    """include/dedisp.h conventions: after dedisp_plan_reserve, dedisp_execute only
+    enqueues on the caller's stream.  A one-second spin kernel is queued on a side stream, then two
+    executes: both calls return while the stream is still busy (cudaStreamQuery != cudaSuccess), the
+    device allocator is untouched between them, and the result is right once the stream drains.  Without
+    a covering reservation execute refuses (DEDISP_ESTATE) instead of allocating."""
+    cf = synth.scaled(synth.configs()[1], dtype="u8", ndm=48, n_out=8192)
+    tab, x = make_case(oracle, cf)
+    plan = dd.Plan(**cf.plan_args())
+    xd = to_dev(x[0])
+    out = torch.empty((cf.ndm, cf.n_out), dtype=torch.int32, device="cuda")
+    L = dd.lib()
+    st = L.dedisp_execute(plan._h, xd.data_ptr(), out.data_ptr(), dd.U8, cf.n_out, xd.stride(0), cf.n_out, 1, 0)
+    assert st == dd.binding.ESTATE                                   # no reservation: no lazy allocation
+    plan.reserve(dd.U8, cf.n_out, 1)
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    with torch.cuda.stream(side):
+        torch.cuda._sleep(2_000_000_000)                             # about a second of device time
+        for _ in range(2):
+            st = L.dedisp_execute(plan._h, xd.data_ptr(), out.data_ptr(), dd.U8, cf.n_out, xd.stride(0), cf.n_out, 1,
+                                  side.cuda_stream)
+            assert st == dd.binding.OK
+            assert not side.query()                                  # returned with the stream still busy
+    assert torch.cuda.mem_get_info()[0] == free0                     # nothing allocated or freed by execute
+    side.synchronize()
+    assert (out.cpu().numpy() == oracle.brute_u8(x[0], tab, cf.n_out)).all()
+    st = L.dedisp_execute(plan._h, xd.data_ptr(), out.data_ptr(), dd.U8, 2 * cf.n_out, xd.stride(0), 2 * cf.n_out, 1, 0)
+    assert st in (dd.binding.ESTATE, dd.binding.ESHAPE)              # beyond the reservation / the input
