@@ -135,7 +135,10 @@ DEDISP_API dedisp_status dedisp_plan_get_subband_shifts(const dedisp_plan *plan,
  * value, DEDISP_ESTATE if WINDOW is forced on a plan whose table exceeds its limits. */
 DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel kernel);
 
-/* Which kernel AUTO resolves to for this plan and dtype (a dedisp_kernel value), -1 on error. */
+/* Which kernel AUTO resolves to for this plan and dtype (a dedisp_kernel value), -1 on error.  This is
+ * the choice for problems that fill the device; an execute whose (trials x samples x beams) yields fewer
+ * register-window tiles than the device has SMs runs the naive kernel (below 8192 outputs per SM) or the
+ * direct kernel instead. */
 DEDISP_API int dedisp_plan_resolved_kernel(const dedisp_plan *plan, dedisp_dtype dtype);
 
 /* Geometry the register-window kernel would use for this plan, 12 int64 to HOST memory:

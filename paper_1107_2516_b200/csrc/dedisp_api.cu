@@ -348,7 +348,15 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     pr.nb0 = nbeams;
     pr.in_len = nsamp_out + plan->max_delay;  // the extent seen from `in`: nothing beyond it is read
     int rc = 0;
-    if (use_window(plan, dtype, nsamp_out))
+    // AUTO looks at the size: tiles of the register-window kernel are 24 rows x ~1900 samples, and a
+    // problem that yields fewer of them than there are SMs (BASELINE cfg 1: 15) is launch- and
+    // latency-bound.  There one thread per output (the paper's own scheme) wins up to
+    // ~8192 outputs per SM, the direct kernel's 8..32 rows x 256 samples beyond (measured on cfg 1:
+    // naive 0.037 ms, direct 0.054 ms, window 0.069 ms, long 0.078 ms).
+    bool small = false;
+    if (plan->kernel == DEDISP_KERNEL_AUTO && plan->nsub == 0 && !sr && use_window(plan, dtype, nsamp_out))
+        small = static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nsamp_out) * nbeams < plan->nsm;
+    if (!small && use_window(plan, dtype, nsamp_out))
         return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream, sr);
     if (sr)
         return DEDISP_ESTATE;  // callers check fused_stats_ok first
@@ -381,7 +389,13 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
         pr.nchans = plan->nchans;
         pr.ndm = plan->ndm;
         pr.nb1 = 1;
-        rc = run_problem(plan, pr, in_t, plan->spread_full, stream);
+        if (small) {
+            const bool tiny = static_cast<int64_t>(plan->ndm) * nsamp_out * nbeams < 8192LL * plan->nsm;
+            rc = tiny ? launch_naive(pr, in_t, stream, &plan->last_launches)
+                      : launch_direct(pr, in_t, plan->spread_full, stream, &plan->last_launches);
+        } else {
+            rc = run_problem(plan, pr, in_t, plan->spread_full, stream);
+        }
         return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
     }
 

@@ -11,7 +11,7 @@ torch = pytest.importorskip("torch")
 pytestmark = pytest.mark.gpu
 
 KERNELS = {"naive": dd.KERNEL_NAIVE, "direct": dd.KERNEL_DIRECT, "auto": dd.KERNEL_AUTO,
-           "long": dd.KERNEL_LONG}
+           "long": dd.KERNEL_LONG, "window": dd.KERNEL_WINDOW}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -71,7 +71,7 @@ def test_brute_small_ragged(oracle, kernel, dtype):
             check_f32(got[b], ref, sa)
 
 
-@pytest.mark.parametrize("kernel", ["direct", "auto"])
+@pytest.mark.parametrize("kernel", ["direct", "auto", "window"])
 def test_cfg1_full(oracle, kernel):
     cf = synth.configs()[1]
     tab, x = make_case(oracle, cf)
@@ -106,6 +106,17 @@ def test_scaled_configs(oracle, k, ndm, n_out):
         assert (got == oracle.brute_u8(x, tab, n_out)).all()
     else:
         ref, sa = oracle.brute_f32(x, tab, n_out)
+        check_f32(got, ref, sa)
+    # the register-window kernel itself on the contiguous top half of the list (the jump in the middle of
+    # `rows` is outside its limits, and AUTO sends a problem this small to the direct kernel anyway)
+    top = dd.Plan(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, dm[ndm // 2:])
+    assert top.window_info()["ok"] == 1
+    top.set_kernel(dd.KERNEL_WINDOW)
+    got = top.execute(to_dev(x), n_out).cpu().numpy()
+    if cf.dtype == "u8":
+        assert (got == oracle.brute_u8(x, tab[ndm // 2:], n_out)).all()
+    else:
+        ref, sa = oracle.brute_f32(x, tab[ndm // 2:], n_out)
         check_f32(got, ref, sa)
 
 
@@ -382,8 +393,10 @@ def test_cfg4_geometry_subband_scaled(oracle):
 
 @pytest.mark.parametrize("chunk_rel", ["larger", "smaller"])
 @pytest.mark.parametrize("dtype", ["u8", "f32"])
-def test_streaming_equals_one_shot(oracle, dtype, chunk_rel):
-    cf = small_cfg(dtype, nchans=64, ndm=40, n_out=0, step=0.3)
+@pytest.mark.parametrize("kernel", ["auto", "window"])
+def test_streaming_equals_one_shot(oracle, dtype, chunk_rel, kernel):
+    cf = small_cfg(dtype, nchans=64, ndm=40, n_out=0, step=0.3) if kernel == "auto" else \
+        synth.scaled(synth.configs()[1], dtype=dtype, nchans=64, ndm=40, n_out=0)
     tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, cf.dm_list)
     M = int(tab.max())
     C = (M + 200) // 4 * 4 if chunk_rel == "larger" else max(16, (M // 3) // 4 * 4)
@@ -392,6 +405,7 @@ def test_streaming_equals_one_shot(oracle, dtype, chunk_rel):
     xs = np.stack([synth.make_input(cf, total, [(7, M + 10, 12, 2.0)], {7: tab[7]}, beam=b)
                    for b in range(beams)])
     plan = dd.Plan(**cf.plan_args())
+    plan.set_kernel(KERNELS[kernel])
     st = dd.Stream(plan, dd.U8 if dtype == "u8" else dd.F32, C, beams)
     outs = []
     for k in range(npush):
