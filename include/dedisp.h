@@ -152,8 +152,8 @@ DEDISP_API dedisp_status dedisp_plan_window_info(const dedisp_plan *plan, int64_
 
 /* Tuning knob: thread / block shape of the register-window kernel.  A thread owns D DM rows x T
  * sample pairs, a block G row groups x NT warps along time.  Only the instantiated shapes are
- * accepted (DEDISP_EINVAL otherwise): (T,G,NT,D) = (15,6,2,4) [default], (15,4,3,4), (21,4,1,4),
- * (21,8,1,4), (17,4,1,5), (15,4,1,6), (11,8,1,8).  Brute-force plans, before the first
+ * accepted (DEDISP_EINVAL otherwise): (T,G,NT,D) = (15,4,3,4) [default where it fits], (15,6,2,4), (21,4,1,4),
+ * (21,8,1,4), (17,4,1,5), (15,4,1,6), (11,6,2,5), (9,6,2,6).  Brute-force plans, before the first
  * dedisp_plan_reserve (DEDISP_ESTATE otherwise, or when the table does not fit the shape: the
  * plan then keeps the shape it had).  Results do not depend on it beyond fp32 summation order. */
 DEDISP_API dedisp_status dedisp_plan_set_window_geometry(dedisp_plan *plan, int T, int G, int NT, int D);

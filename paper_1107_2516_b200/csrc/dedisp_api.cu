@@ -94,7 +94,7 @@ struct dedisp_plan {
     // register-window kernel (brute-force plans): host plan, device tables, pair scratch
     WindowPlan win;
     bool win_fits = false;
-    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr, *d_win_theta = nullptr, *d_win_hdr = nullptr;
+    int32_t *d_win_meta = nullptr, *d_win_kfinal = nullptr, *d_win_theta = nullptr, *d_win_hdr = nullptr, *d_win_first = nullptr;
     void* d_win_zeros = nullptr;
     DevBuf pairs;
     // optional timing of the dominant kernel(s) of an execute (dedisp_plan_set_timing)
@@ -137,7 +137,7 @@ size_t in_size(dedisp_dtype t) { return t == DEDISP_F32 ? 4 : 1; }
 void free_tables(dedisp_plan* p)
 {
     int32_t** tabs[] = {&p->d_shift, &p->d_s1, &p->d_s2, &p->d_maxshift2, &p->d_maxshift2_ks,
-                        &p->d_win_meta, &p->d_win_kfinal, &p->d_win_theta, &p->d_win_hdr};
+                        &p->d_win_meta, &p->d_win_kfinal, &p->d_win_theta, &p->d_win_hdr, &p->d_win_first};
     for (int32_t** t : tabs) {
         if (*t)
             cudaFree(*t);
@@ -178,6 +178,8 @@ dedisp_status upload(dedisp_plan* p)
                 e = up(&p->d_win_theta, p->win.theta);
             if (e == cudaSuccess)
                 e = up(&p->d_win_hdr, p->win.hdr);
+            if (e == cudaSuccess)
+                e = up(&p->d_win_first, p->win.first);
             if (e == cudaSuccess) {
                 const size_t zb = static_cast<size_t>(p->win.lmax + 16) * 8;
                 e = cudaMalloc(&p->d_win_zeros, zb);
@@ -250,6 +252,7 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.kfinal = plan->d_win_kfinal;
     a.theta = plan->d_win_theta;
     a.hdr = plan->d_win_hdr;
+    a.first = plan->d_win_first;
     a.zeros = plan->d_win_zeros;
     a.stage0 = plan->win.stage0.data();
     a.stage_total = plan->win.stage0[plan->win.nband];
@@ -543,8 +546,12 @@ dedisp_status dedisp_plan_create(dedisp_plan** plan, int nchans, double f_top_mh
         if (nsub == 0) {
             for (int k = 0; k < 3; ++k)
                 p->spread_full[k] = tile_spread(p->shift.data(), ndm, nchans, nchans, tiles[k]);
-            build_window_plan(p->shift.data(), ndm, nchans, window_default_geom(), p->win);
-            p->win_fits = p->win.ok && window_fits_smem(p->win);
+            WindowGeom pref[4];
+            const int npref = window_geom_preferences(pref, 4);
+            for (int k = 0; k < npref && !p->win_fits; ++k) {
+                build_window_plan(p->shift.data(), ndm, nchans, pref[k], p->win);
+                p->win_fits = p->win.ok && window_fits_smem(p->win);
+            }
         } else {
             build_subband_tables(p->shift, nchans, ndm, nsub, nfine, dm_list, p->s1, p->s2, p->nominal,
                                  p->maxshift2, p->max_delay);

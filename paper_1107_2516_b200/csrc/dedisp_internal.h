@@ -80,9 +80,11 @@ int launch_fadd_microbench(int packed, int iters, int nsm, float* sink, void* st
 // row group; lane L owns the T consecutive "slots" L*T .. L*T+T-1 of each row, a slot being one
 // pair of output samples (t, t + NT*W).  A block has G row groups x NT warps along time
 // (+ 1 producer warp); the channel loop is cut into bands, one launch per band.
-constexpr int kWinD = 8;            // most DM rows per thread (metadata word: 7 bits per mask)
+constexpr int kWinD = 6;            // most DM rows per thread (metadata word: 5 bits per mask)
 constexpr int kWinMetaWords = 16;   // per (DM tile, channel) metadata, 64 bytes
 constexpr int kWinWbBits = 11;
+constexpr unsigned kWinShiftBits = 0x7fe0u;   // bits 5..14 of a channel word: the two row-shift masks
+constexpr unsigned kWinStageShift = 0x8000u;  // bit 15: some channel of the stage this channel opens has a row shift
 constexpr int kWinCh = 4;           // channels per pipeline stage (one mbarrier pair per stage)
 constexpr int kWinHdrWords = 32;    // per (DM tile, stage) header: [row group][kWinCh] words, 128 bytes      // window offset inside the staged segment, in pairs
 
@@ -107,11 +109,15 @@ struct WindowPlan {
     int64_t maxbase = 0;        // largest staged-segment start (pairs, relative to the tile start)
     std::vector<int32_t> band;  // [nband + 1] channel boundaries
     // meta[tile][c] = { base, len, m[G], 0.. }: staged segment start / length in pairs (both even)
-    // and, per row group, jitter bits (rows 1..7) | shift mask << 7 | 2nd shift mask << 14 |
-    // window offset << 21
+    // and, per row group, the channel's word: jitter bits (rows 1..5) | shift mask << 5 | 2nd shift
+    // mask << 10 | kWinStageShift if a channel of the 4-channel stage this channel opens has a row
+    // shift | window offset << 21
     std::vector<int32_t> meta;
     std::vector<int32_t> stage0;  // [nband + 1] first stage of every band in hdr
+    // hdr[tile][stage][g * kWinCh + ch] = word of the channel AFTER channel ch of that stage (0 past the
+    // band's end): a consumer reads the next channel's word from the stage it is working on
     std::vector<int32_t> hdr;     // [tile][stage0[nband]][kWinHdrWords]
+    std::vector<int32_t> first;   // [tile][band][G] word of the band's first channel
     std::vector<int32_t> kfinal;  // [tile][band][rows] row shifts of every row at the band's end
     std::vector<int32_t> theta;   // [tile][band][rows] band skew of every row
 };
@@ -133,6 +139,7 @@ struct WindowArgs {
     const int32_t* band;    // HOST pointer, [nband + 1]
     const int32_t* stage0;  // HOST pointer, [nband + 1]
     const int32_t* hdr;     // device copy of WindowPlan::hdr
+    const int32_t* first;   // device copy of WindowPlan::first
     const void* zeros;      // device, >= lmax pairs of zeros (segments of the padding channels)
     WindowGeom geom;
     // fused statistics of the outputs (band 0 of single-band plans only): per beam a pivot, per block two
@@ -147,6 +154,7 @@ int64_t window_ntile_t(const WindowPlan& wp, int64_t n_out);
 int64_t window_pair_stride(const WindowPlan& wp, int64_t n_out);  // float2 elements per channel row
 int launch_window(const WindowArgs& a, Elem in_t, void* stream, int* launches);
 WindowGeom window_default_geom();
+int window_geom_preferences(WindowGeom* g, int max);  // shapes to try at plan creation, best first
 bool window_geom_supported(const WindowGeom& g);  // one of the instantiated kernels
 
 }  // namespace dedisp

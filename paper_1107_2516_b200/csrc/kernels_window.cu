@@ -93,6 +93,12 @@ __device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+__device__ __forceinline__ unsigned lds32(unsigned addr)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
 // producer side: the staging thread shares its scheduler with two consumer warps, so it must not
 // spin: try_wait with a suspend-time hint parks the thread in hardware between polls
 __device__ __forceinline__ void mbar_wait_backoff(unsigned bar, unsigned parity)
@@ -364,22 +370,24 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // added (wa / wb alternate).
     const unsigned lane_off = kWinHdrWords * 4 + (wt * W + lane_pinned * T) * 8;  // bytes from the slot start
     auto shifts = [&](unsigned m) {
-        const unsigned sm = (m >> 7) & 0x3fffu;
-        shift_rows<T, D, OutT>(acc, sm & 127u, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
-        if (sm >> 7)
-            shift_rows<T, D, OutT>(acc, sm >> 7, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
+        const unsigned sm = (m >> 5) & 0x3ffu;
+        shift_rows<T, D, OutT>(acc, sm & 31u, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
+        if (sm >> 5)
+            shift_rows<T, D, OutT>(acc, sm >> 5, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
     };
     auto adds = [&](u64(&w)[T + 1], unsigned m) { rows7(acc, w, m); };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
-    // accumulator registers between copies otherwise).  The bookkeeping that runs once per channel
-    // is kept to the window address and the rotation of the stage's four metadata words: every
-    // uniform-datapath instruction in that chain costs its full latency with two warps per scheduler.
-    // The next stage's barrier wait and metadata load sit between two stages, outside the channel
-    // loop: three more bookkeeping instructions per channel cost more than the exposed latency.
+    // accumulator registers between copies otherwise).  A warp carries the current channel's word m in a
+    // uniform register; the NEXT channel's word is read from the stage's header at the top of the
+    // iteration, next to the window loads, and moved into m after the adds, so its latency never shows
+    // and a stage boundary is nothing but the barrier traffic (arrive, wait for the next stage).  Every
+    // uniform-datapath instruction in the per-channel chain costs its full latency with three warps per
+    // scheduler, so that chain is kept to the window address.
     u64 w[T + 1];
-    const unsigned hdr_off = 16 * g;
+    const unsigned hdr_off = 4 * kWinCh * g;
+    unsigned m = __ldg(a.first + (static_cast<int64_t>(ty) * a.nband + band) * G + g);
+    m = __reduce_or_sync(0xffffffffu, m);   // warp-uniform by construction; this lets ptxas know
     mbar_wait(bar_full, 0);
-    uint4 mq = *reinterpret_cast<const uint4*>(stages + hdr_off);
     const unsigned char* sbase = stages;
     int ring = 0;
     unsigned par = 0;
@@ -391,42 +399,39 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             ring_n = 0;
             par_n ^= 1u;
         }
-        const unsigned char* sbase_n = stages + ring_n * stage_bytes;
         const unsigned char* sp = sbase + lane_off;
-        unsigned m = mq.x;
-        if (((mq.x | mq.y) | (mq.z | mq.w)) & 0x1fff80u) {
+        unsigned hw = smem_u32(sbase) + hdr_off;   // this row group's words of the channels one further on
+        if (m & kWinStageShift) {
             // a row shift somewhere in this stage (about a third of the stages)
 #pragma unroll 1
             for (int ch = 0; ch < kWinCh; ++ch) {
+                const unsigned mn = lds32(hw);
                 load_window<T>(w, sp + (m >> 21) * 8);
-                if (m & 0x1fff80u)
+                if (m & kWinShiftBits)
                     shifts(m);
                 adds(w, m);
                 sp += slot_bytes;
-                m = mq.y;
-                mq.y = mq.z;
-                mq.z = mq.w;
+                hw += 4;
+                m = mn;
             }
         } else {
 #pragma unroll 1
             for (int ch = 0; ch < kWinCh; ++ch) {
+                const unsigned mn = lds32(hw);
                 load_window<T>(w, sp + (m >> 21) * 8);
                 adds(w, m);
                 sp += slot_bytes;
-                m = mq.y;
-                mq.y = mq.z;
-                mq.z = mq.w;
+                hw += 4;
+                m = mn;
             }
         }
         __syncwarp();
         mbar_arrive_one(bar_empty + 8u * ring);
-        if (s + 1 < nstage) {
+        if (s + 1 < nstage)
             mbar_wait(bar_full + 8u * ring_n, par_n);
-            mq = *reinterpret_cast<const uint4*>(sbase_n + hdr_off);
-        }
         ring = ring_n;
         par = par_n;
-        sbase = sbase_n;
+        sbase = stages + ring_n * stage_bytes;
     }
 
     // ---- flush ------------------------------------------------------------------------------------------
@@ -647,7 +652,7 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
 }
 
 // instantiated geometries: (T, G, NT, D)
-#define DEDISP_GEOMS(X) X(15, 6, 2, 4) X(15, 4, 3, 4) X(21, 4, 1, 4) X(21, 8, 1, 4) X(17, 4, 1, 5) X(15, 4, 1, 6) X(11, 8, 1, 8) \
+#define DEDISP_GEOMS(X) X(15, 6, 2, 4) X(15, 4, 3, 4) X(21, 4, 1, 4) X(21, 8, 1, 4) X(17, 4, 1, 5) X(15, 4, 1, 6) \
     X(11, 6, 2, 5) X(9, 6, 2, 6)
 
 template <typename OutT> static int launch_geom(const WindowArgs& a, cudaStream_t st, int* launches)

@@ -27,17 +27,31 @@
 
 namespace dedisp {
 
+// Preference order of the thread / block shapes at plan creation: 4 rows x 15 pairs per thread, 12 consumer
+// warps (three per scheduler, 160 registers each) in one block per SM.  Three warps along time (NT = 3,
+// G = 4 row groups) lose kmax samples per 6 warp segments and measured best on cfg 2, 3 and 5; two warps
+// along time with 6 row groups stage shorter channel segments and take over when the NT = 3 ring does not
+// fit shared memory.
+int window_geom_preferences(WindowGeom* g, int max)
+{
+    static const int pref[][4] = {{15, 4, 3, 4}, {15, 6, 2, 4}, {21, 8, 1, 4}};
+    int n = 0;
+    for (const auto& p : pref) {
+        if (n == max)
+            break;
+        g[n].T = p[0];
+        g[n].G = p[1];
+        g[n].NT = p[2];
+        g[n].D = p[3];
+        ++n;
+    }
+    return n;
+}
+
 WindowGeom window_default_geom()
 {
     WindowGeom g;
-    // 4 rows x 15 pairs per thread, 6 row groups x 2 warps along time = 12 consumer warps (three per
-    // scheduler, 160 registers each) in one block per SM.  4 rows instead of 8: fewer row variants
-    // (branches) per add and a slower drift between a thread's rows, so fewer bands.  4 x 21 pairs with
-    // 8 consumer warps (21,4,1,4) is within 2 % (better on cfg 2, worse on cfg 3 and cfg 5).
-    g.T = 15;
-    g.G = 6;
-    g.NT = 2;
-    g.D = 4;
+    window_geom_preferences(&g, 1);
     return g;
 }
 
@@ -191,9 +205,9 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
                         if (o)
                             word |= 1u << (j - 1);
                         if (ns >= 1)
-                            word |= 1u << (7 + j - 1);
+                            word |= 1u << (5 + j - 1);
                         if (ns >= 2)
-                            word |= 1u << (14 + j - 1);
+                            word |= 1u << (10 + j - 1);
                     }
                     m[2 + g] = static_cast<int32_t>(word);
                 }
@@ -207,24 +221,41 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
             }
         }
     }
-    // ---- stage headers: the kernel consumes kWinCh channels per barrier; the words of those channels
-    // are regrouped per row group (hdr[g * kWinCh + ch]) so that a warp reads them with one LDS.128.
-    // Channels past the band's end and one extra stage per band stay zero (the kernel stages a
-    // zero segment for them).
+    // ---- stage headers: the kernel consumes kWinCh channels per barrier.  A consumer warp carries the
+    // current channel's word in a (uniform) register and reads the NEXT channel's word while it adds, so
+    // the header of a stage holds, regrouped per row group (hdr[g * kWinCh + ch]), the words of the
+    // channels one further on; the band's first word comes from `first`.  The word of a channel that
+    // opens a stage says whether any channel of that stage has a row shift (the kernel then runs the
+    // loop variant that tests for shifts).  Channels past the band's end and one extra stage per band
+    // stay zero (the kernel stages a zero segment for them).
     wp.stage0.assign(wp.nband + 1, 0);
     for (int b = 0; b < wp.nband; ++b)
         wp.stage0[b + 1] = wp.stage0[b] + (wp.band[b + 1] - wp.band[b] + kWinCh - 1) / kWinCh + 1;
     const int nst = wp.stage0[wp.nband];
     wp.hdr.assign(static_cast<size_t>(ntile) * nst * kWinHdrWords, 0);
+    wp.first.assign(static_cast<size_t>(ntile) * wp.nband * G, 0);
     for (int ty = 0; ty < ntile; ++ty)
-        for (int b = 0; b < wp.nband; ++b)
-            for (int c = wp.band[b]; c < wp.band[b + 1]; ++c) {
-                const int s = wp.stage0[b] + (c - wp.band[b]) / kWinCh, ch = (c - wp.band[b]) % kWinCh;
-                const int32_t* m = wp.meta.data() + (static_cast<size_t>(ty) * nchans + c) * kWinMetaWords;
-                int32_t* h = wp.hdr.data() + (static_cast<size_t>(ty) * nst + s) * kWinHdrWords;
-                for (int g = 0; g < G; ++g)
-                    h[g * kWinCh + ch] = m[2 + g];
+        for (int b = 0; b < wp.nband; ++b) {
+            const int c0 = wp.band[b], c1 = wp.band[b + 1];
+            for (int g = 0; g < G; ++g) {
+                auto word_of = [&](int c) -> uint32_t& {
+                    return reinterpret_cast<uint32_t&>(wp.meta[(static_cast<size_t>(ty) * nchans + c) * kWinMetaWords + 2 + g]);
+                };
+                for (int cs = c0; cs < c1; cs += kWinCh) {
+                    bool any = false;
+                    for (int c = cs; c < std::min(cs + kWinCh, c1); ++c)
+                        any = any || (word_of(c) & kWinShiftBits) != 0;
+                    if (any)
+                        word_of(cs) |= kWinStageShift;
+                }
+                wp.first[(static_cast<size_t>(ty) * wp.nband + b) * G + g] = static_cast<int32_t>(word_of(c0));
+                for (int c = c0; c + 1 < c1; ++c) {
+                    const int s = wp.stage0[b] + (c - c0) / kWinCh, ch = (c - c0) % kWinCh;
+                    wp.hdr[(static_cast<size_t>(ty) * nst + s) * kWinHdrWords + g * kWinCh + ch] =
+                        static_cast<int32_t>(word_of(c + 1));
+                }
             }
+        }
     wp.lmax = lmax;
     wp.maxbase = maxbase;
     wp.theta_max = theta_max;

@@ -147,16 +147,15 @@ def test_window_kernel_forced(oracle, dtype, beams, n_out, nchans):
     assert (again == got).all()
 
 
-GEOMS = [(15, 6, 2, 4), (15, 4, 3, 4), (21, 4, 1, 4), (21, 8, 1, 4), (17, 4, 1, 5), (15, 4, 1, 6), (11, 8, 1, 8),
-         (11, 6, 2, 5), (9, 6, 2, 6)]
+GEOMS = [(15, 6, 2, 4), (15, 4, 3, 4), (21, 4, 1, 4), (21, 8, 1, 4), (17, 4, 1, 5), (15, 4, 1, 6), (11, 6, 2, 5),
+         (9, 6, 2, 6)]
 
 
 @pytest.mark.parametrize("geom", GEOMS)
 def test_window_geometries(oracle, geom):
     """Every instantiated thread / block shape of the register-window kernel (dedisp_plan_set_window_geometry)
     on the cfg-2 band with 1024 channels: rows drift by tens of slots, so the hand-over of partial sums
-    between warp segments, several blocks along time and (for the 8-row shapes) several channel bands are
-    all exercised; uint8 bit-exact, two beams, an output length that ends inside a block."""
+    between warp segments and several blocks along time are exercised; uint8 bit-exact, two beams, an output length that ends inside a block."""
     T, G, NT, D = geom
     cf = synth.scaled(synth.configs()[2], dtype="u8", n_out=3 * 2 * NT * 32 * T + 777, ndm=2 * D * G + 3, nchans=1024)
     tab, x = make_case(oracle, cf, beams=2)
