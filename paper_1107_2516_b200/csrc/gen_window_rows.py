@@ -60,6 +60,60 @@ def rows7(T, D=8):
             "{\n    asm volatile(\n%s\n        : %s\n        : %s, \"r\"(m));\n}\n" % (D, T, T + 1, body, outs, ins))
 
 
+def chan_loop(T, D):
+    """The whole per-channel loop of a stage as ONE asm statement of threaded code:
+
+        chan_loop(acc, m, hw, sp, ch, slot_bytes)
+
+    m = word of the current channel, hw = shared-memory address of the next channel's word, sp = this
+    thread's window base in the current channel's slot, ch = channels left in the stage.  Per channel:
+    next word (ld.shared), T + 1 window loads, row 0, then ONE indirect branch (brx.idx over the
+    2^(D-1) offset patterns of rows 1 .. D-1) into a straight-line block that adds the other rows and
+    then does the next channel's loads and row 0 ITSELF before branching on: a channel costs exactly one
+    taken branch (the two-chain version of rows7 takes two on average; forcing all offsets to 0 in an
+    experiment, i.e. one taken branch fewer per channel, made the kernel 13 % faster).  Measured: 1.3 % over
+    the chains for 4 rows (8 variants of ~1.4 KB), nothing for 5, much slower for 6 rows (32 variants no
+    longer sit in the instruction cache), and a compact form with a shared tail is slower than either.  Leaves when the stage is done (ch == 0) or when the next channel has a row shift
+    (m & SHIFT != 0: the caller shifts, clears those bits and comes back)."""
+    NP = 1 << (D - 1)
+    NA = D * T
+    M, HW, SP, CH, SB = NA, NA + 1, NA + 2, NA + 3, NA + 4
+    L = ["{ .reg .b64 w<%d>; .reg .b32 mn, t, a, idx; .reg .pred pe, ps;" % (T + 1)]
+
+    def adds(row, o):
+        return ["add.rn.f32x2 %%%d, %%%d, w%d;" % (row * T + i, row * T + i, i + o) for i in range(T)]
+
+    def top(tag):
+        # loads and row 0 of the channel whose word is m; exits first if it needs a row shift
+        X = ["and.b32 t, %%%d, %d; setp.ne.u32 ps, t, 0; @ps bra.uni DONE_%%=;" % (M, 0x7fe0)]
+        X.append("ld.shared.u32 mn, [%%%d];" % HW)
+        X.append("shr.u32 t, %%%d, 21; shl.b32 t, t, 3; add.u32 a, %%%d, t;" % (M, SP))
+        X += ["ld.shared.b64 w%d, [a+%d];" % (k, 8 * k) for k in range(T + 1)]
+        X.append("and.b32 idx, %%%d, %d;" % (M, NP - 1))
+        X += adds(0, 0)
+        X.append("brx.idx.uni idx, TS_%=;")
+        return X
+
+    L.append("TS_%=: .branchtargets " + ", ".join("V%d_%%=" % p for p in range(NP)) + ";")
+    L.append("setp.eq.u32 pe, %%%d, 0; @pe bra.uni DONE_%%=;" % CH)
+    L += top("entry")
+    for p in range(NP):
+        L.append("V%d_%%=:" % p)
+        for r in range(1, D):
+            L += adds(r, (p >> (r - 1)) & 1)
+        L.append("mov.b32 %%%d, mn; add.u32 %%%d, %%%d, 4; add.u32 %%%d, %%%d, %%%d; sub.u32 %%%d, %%%d, 1;"
+                 % (M, HW, HW, SP, SP, SB, CH, CH))
+        L.append("setp.eq.u32 pe, %%%d, 0; @pe bra.uni DONE_%%=;" % CH)
+        L += top("v%d" % p)
+    L.append("DONE_%=:")
+    L.append("}")
+    body = "\n".join('        "%s\\n"' % x for x in L)
+    outs = ", ".join('"+l"(acc[%d][%d])' % (r, i) for r in range(D) for i in range(T))
+    return ("__device__ __forceinline__ void chan_loop(u64 (&acc)[%d][%d], unsigned& m, unsigned& hw, unsigned& sp, unsigned& ch, unsigned slot_bytes)\n"
+            "{\n    asm volatile(\n%s\n        : %s, \"+r\"(m), \"+r\"(hw), \"+r\"(sp), \"+r\"(ch)\n        : \"r\"(slot_bytes)\n        : \"memory\");\n}\n"
+            % (D, T, body, outs))
+
+
 def shift_row(T):
     """a[i] = a[i-1] (i = T-1 .. 1), a[0] = carry, as exact adds of -0.0 on tied operands: with plain
     copies or untied outputs ptxas rotates the accumulator registers inside the hot loop."""
@@ -79,6 +133,8 @@ def main():
     out = ["// GENERATED by gen_window_rows.py -- do not edit.\n"]
     for D, T in COMBOS:
         out.append(rows7(T, D))
+        if D == 4:  # 8 variants; with 5 rows (16) it is no faster than the chains, with 6 (32) far slower (I-cache)
+            out.append(chan_loop(T, D))
     for T in sorted({t for _, t in COMBOS}):
         out.append(shift_row(T))
     with open(os.path.join(here, "window_rows.inc"), "w") as f:

@@ -375,7 +375,6 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
         if (sm >> 5)
             shift_rows<T, D, OutT>(acc, sm >> 5, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
     };
-    auto adds = [&](u64(&w)[T + 1], unsigned m) { rows7(acc, w, m); };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
     // accumulator registers between copies otherwise).  A warp carries the current channel's word m in a
     // uniform register; the NEXT channel's word is read from the stage's header at the top of the
@@ -383,7 +382,6 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // and a stage boundary is nothing but the barrier traffic (arrive, wait for the next stage).  Every
     // uniform-datapath instruction in the per-channel chain costs its full latency with three warps per
     // scheduler, so that chain is kept to the window address.
-    u64 w[T + 1];
     const unsigned hdr_off = 4 * kWinCh * g;
     unsigned m = __ldg(a.first + (static_cast<int64_t>(ty) * a.nband + band) * G + g);
     m = __reduce_or_sync(0xffffffffu, m);   // warp-uniform by construction; this lets ptxas know
@@ -399,30 +397,47 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             ring_n = 0;
             par_n ^= 1u;
         }
-        const unsigned char* sp = sbase + lane_off;
-        unsigned hw = smem_u32(sbase) + hdr_off;   // this row group's words of the channels one further on
-        if (m & kWinStageShift) {
-            // a row shift somewhere in this stage (about a third of the stages)
-#pragma unroll 1
-            for (int ch = 0; ch < kWinCh; ++ch) {
-                const unsigned mn = lds32(hw);
-                load_window<T>(w, sp + (m >> 21) * 8);
-                if (m & kWinShiftBits)
-                    shifts(m);
-                adds(w, m);
-                sp += slot_bytes;
-                hw += 4;
-                m = mn;
+        unsigned hw = smem_u32(sbase) + hdr_off;    // this row group's words of the channels one further on
+        if constexpr (D == 4) {
+            // threaded code (window_rows.inc, chan_loop): one indirect branch per channel over the 8 offset
+            // patterns; runs channels until the stage is done or one needs a row shift
+            unsigned spa = smem_u32(sbase) + lane_off;  // this thread's window base in the stage's first slot
+            unsigned chn = kWinCh;
+            while (true) {
+                chan_loop(acc, m, hw, spa, chn, static_cast<unsigned>(slot_bytes));
+                if (chn == 0)
+                    break;
+                shifts(m);
+                m &= ~kWinShiftBits;
             }
         } else {
+            // two chains of row blocks (rows7), one uniform branch per row whose offset differs from the
+            // previous row's
+            u64 w[T + 1];
+            const unsigned char* sp = sbase + lane_off;
+            if (m & kWinStageShift) {
+                // a row shift somewhere in this stage (about a third of the stages)
 #pragma unroll 1
-            for (int ch = 0; ch < kWinCh; ++ch) {
-                const unsigned mn = lds32(hw);
-                load_window<T>(w, sp + (m >> 21) * 8);
-                adds(w, m);
-                sp += slot_bytes;
-                hw += 4;
-                m = mn;
+                for (int ch = 0; ch < kWinCh; ++ch) {
+                    const unsigned mn = lds32(hw);
+                    load_window<T>(w, sp + (m >> 21) * 8);
+                    if (m & kWinShiftBits)
+                        shifts(m);
+                    rows7(acc, w, m);
+                    sp += slot_bytes;
+                    hw += 4;
+                    m = mn;
+                }
+            } else {
+#pragma unroll 1
+                for (int ch = 0; ch < kWinCh; ++ch) {
+                    const unsigned mn = lds32(hw);
+                    load_window<T>(w, sp + (m >> 21) * 8);
+                    rows7(acc, w, m);
+                    sp += slot_bytes;
+                    hw += 4;
+                    m = mn;
+                }
             }
         }
         __syncwarp();
