@@ -183,6 +183,35 @@ def test_window_geometries(oracle, geom):
         p2.set_window_geometry(13, 5, 2, 4)            # not an instantiated shape
 
 
+@pytest.mark.parametrize("dtype", ["u8", "f32"])
+def test_window_kernel_several_channel_bands(oracle, dtype):
+    """A table whose rows drift too fast for one channel band (cfg-2 band, twice its DM step, 6 rows per
+    thread): the register-window kernel runs three launches; bands after the first ADD to the output, and
+    their hand-over of partial sums goes through red.global.add on both sides.  Every output against the
+    oracle; a second execute on the same buffer must not accumulate on the first."""
+    cf = synth.scaled(synth.configs()[2], dtype=dtype, dm_step=0.1, ndm=2 * 36 + 5, nchans=1024, n_out=3 * 1100 + 321)
+    tab, x = make_case(oracle, cf, beams=2)
+    plan = dd.Plan(**cf.plan_args())
+    plan.set_window_geometry(9, 6, 2, 6)
+    info = plan.window_info()
+    assert info["ok"] == 1 and info["nband"] >= 2
+    plan.set_kernel(dd.KERNEL_WINDOW)
+    xd = to_dev(x)
+    for rep in range(2):
+        got = plan.execute(xd, cf.n_out).cpu().numpy()
+        assert plan.last_launches == 1 + info["nband"]
+        for b in range(2):
+            if dtype == "u8":
+                assert (got[b] == oracle.brute_u8(x[b], tab, cf.n_out)).all()
+            else:
+                ref, sa = oracle.brute_f32(x[b], tab, cf.n_out)
+                check_f32(got[b], ref, sa)
+    # detection on a multi-band plan takes the unfused route (an output is final only after the last band)
+    out, res, ev = plan.execute_detect(xd, cf.n_out, 4.0)
+    mu, sg, thr, evo, val = oracle.detect(out[0].cpu().numpy(), 4.0)
+    assert res[0]["count"] == len(evo) and abs(res[0]["sigma"] - sg) <= 1e-11 * sg
+
+
 @pytest.mark.parametrize("seed", [1, 2, 3, 4, 5, 6])
 def test_random_plans_all_kernels(oracle, seed):
     """Seeded random bands, sampling times and DM lists (irregular steps, repeated trials, a DM count
