@@ -141,12 +141,13 @@ DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel
  * direct kernel instead. */
 DEDISP_API int dedisp_plan_resolved_kernel(const dedisp_plan *plan, dedisp_dtype dtype);
 
-/* Geometry the register-window kernel would use for this plan, 12 int64 to HOST memory:
+/* Geometry the register-window kernel would use for this plan, 14 int64 to HOST memory:
  * [0] 1 if the plan's table fits the kernel (else the rest is 0), [1] Hb: output samples per
  * block and DM row (blocks are Hb apart in time), [2] kmax: largest number of row shifts in a
  * channel band = samples a block loses, Hb = 2*NT*W - kmax, [3] longest staged channel segment
  * in pairs, [4] DM tiles, [5] W: slots per row and warp segment, [6] DM rows per block,
- * [7] channel bands (= kernel launches), [8] T, [9] G, [10] NT, [11] D (below).
+ * [7] channel bands (= kernel launches), [8] T, [9] G, [10] NT, [11] D (below), [12] channels per
+ * pipeline stage and [13] stages of the shared-memory ring the staged segments go through.
  * Brute-force plans only carry one. */
 DEDISP_API dedisp_status dedisp_plan_window_info(const dedisp_plan *plan, int64_t *info);
 

@@ -180,9 +180,10 @@ class Plan:
 
     def window_info(self):
         """dedisp_plan_window_info as a dict (geometry of the register-window kernel)."""
-        a = np.zeros(12, dtype=np.int64)
+        a = np.zeros(14, dtype=np.int64)
         _check(lib().dedisp_plan_window_info(self._h, a.ctypes.data), "dedisp_plan_window_info")
-        keys = ("ok", "Hb", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "nband", "T", "G", "NT", "D")
+        keys = ("ok", "Hb", "kmax", "lmax", "ntile_dm", "slots", "rows_per_block", "nband", "T", "G", "NT", "D",
+                "stage_channels", "ring_stages")
         return dict(zip(keys, (int(v) for v in a)))
 
     def scratch_bytes(self, nsamp_out, nbeams=1):

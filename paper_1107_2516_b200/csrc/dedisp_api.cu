@@ -280,6 +280,10 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
     a.Hb = plan->win.Hb;
     a.kmax = plan->win.kmax;
     a.lmax = plan->win.lmax;
+    a.ch = plan->win.ch;
+    a.nst = plan->win.nst;
+    a.slot_bytes = plan->win.slot_bytes;
+    a.hdr_words = plan->win.hdr_words;
     a.ntile_dm = plan->win.ntile_dm;
     a.ntile_t = static_cast<int>(window_ntile_t(plan->win, nsamp_out));
     {
@@ -749,6 +753,8 @@ dedisp_status dedisp_plan_window_info(const dedisp_plan* p, int64_t* info)
     info[9] = p->win.geom.G;
     info[10] = p->win.geom.NT;
     info[11] = p->win.geom.D;
+    info[12] = p->win.ch;
+    info[13] = p->win.nst;
     return DEDISP_OK;
 }
 

@@ -85,8 +85,8 @@ constexpr int kWinMetaWords = 16;   // per (DM tile, channel) metadata, 64 bytes
 constexpr int kWinWbBits = 11;
 constexpr unsigned kWinShiftBits = 0x7fe0u;   // bits 5..14 of a channel word: the two row-shift masks
 constexpr unsigned kWinStageShift = 0x8000u;  // bit 15: some channel of the stage this channel opens has a row shift
-constexpr int kWinCh = 4;           // channels per pipeline stage (one mbarrier pair per stage)
-constexpr int kWinHdrWords = 32;    // per (DM tile, stage) header: [row group][kWinCh] words, 128 bytes      // window offset inside the staged segment, in pairs
+constexpr int kWinChMax = 12;       // most channels per pipeline stage (one mbarrier pair per stage)
+constexpr int kWinFixedBytes = 128 + 16 * 128;  // shared memory in front of the ring: barriers + 16 consumer warps' hand-over state
 
 struct WindowGeom {
     int T = 0;   // slots per lane and row (odd: conflict-free LDS.64)
@@ -103,6 +103,9 @@ struct WindowPlan {
     int Hb = 0;         // output samples per block and row: 2 * NT * W - kmax (blocks are Hb samples apart)
     int kmax = 0;       // largest number of row shifts of a row inside one band
     int lmax = 0;       // longest staged channel segment, in pairs
+    // ring of the staged segments (window_ring): ch channels per pipeline stage, nst stages of
+    // { hdr_words header words, ch slots of slot_bytes }; nst = 0: the segments do not fit shared memory
+    int ch = 0, nst = 0, slot_bytes = 0, hdr_words = 0;
     int ntile_dm = 0;
     int nband = 0;
     int theta_max = 0;  // largest band skew of a row
@@ -114,9 +117,9 @@ struct WindowPlan {
     // shift | window offset << 21
     std::vector<int32_t> meta;
     std::vector<int32_t> stage0;  // [nband + 1] first stage of every band in hdr
-    // hdr[tile][stage][g * kWinCh + ch] = word of the channel AFTER channel ch of that stage (0 past the
+    // hdr[tile][stage][g * ch + c] = word of the channel AFTER channel c of that stage (0 past the
     // band's end): a consumer reads the next channel's word from the stage it is working on
-    std::vector<int32_t> hdr;     // [tile][stage0[nband]][kWinHdrWords]
+    std::vector<int32_t> hdr;     // [tile][stage0[nband]][hdr_words]
     std::vector<int32_t> first;   // [tile][band][G] word of the band's first channel
     std::vector<int32_t> kfinal;  // [tile][band][rows] row shifts of every row at the band's end
     std::vector<int32_t> theta;   // [tile][band][rows] band skew of every row
@@ -134,6 +137,7 @@ struct WindowArgs {
     const int32_t* theta;
     int64_t in_stride, out_stride, pair_stride, in_len, n_out;
     int nchans, ndm, nbeams, Hb, kmax, lmax, ntile_dm, ntile_t, nband, stage_total, theta_max;
+    int ch, nst, slot_bytes, hdr_words;  // ring layout (WindowPlan)
     int flush_rows;  // rows per transpose pass of the flush (set by the launcher)
     int dm_group;  // DM tiles per block-order group (kernels_window.cu)
     const int32_t* band;    // HOST pointer, [nband + 1]

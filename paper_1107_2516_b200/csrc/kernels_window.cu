@@ -225,13 +225,13 @@ __device__ __forceinline__ void tile_of(const WindowArgs& a, int lin, int& ty, i
 
 // smem layout: [nst] full barriers | [nst] empty barriers | Fall[NCW] | nst stages of { 128-byte header,
 //              kWinCh channel slots }; the flush's transpose scratch [NCW][W] u64 overlays the stages
-constexpr int kWinFixedBytes = 128 + 16 * kFallBytes;  // barriers + up to 16 consumer warps' Fall
+static_assert(kWinFixedBytes == 128 + 16 * kFallBytes, "barriers + up to 16 consumer warps' hand-over state");
 
 template <int T, int G, int NT, int D, typename OutT>
 __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
-    window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0,
-                  const int nst, const int slot_bytes)
+    window_kernel(const WindowArgs a, const int c_begin, const int c_end, const int band, const int stage0)
 {
+    const int nst = a.nst, slot_bytes = a.slot_bytes, CH = a.ch, hdr_bytes = a.hdr_words * 4;
     constexpr int W = 32 * T, NCW = G * NT, RB = D * G;
     // registers per consumer thread once the producer warp group has released its share
     // (blocks of 4 consumer warps run two to an SM and share the register file)
@@ -255,7 +255,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // the flush's transpose scratch [NCW][W] u64 reuses the ring once every consumer has left the loop
     const int stages_off = kWinFixedBytes;
     const int tr_off = stages_off;
-    const int stage_bytes = kWinHdrWords * 4 + kWinCh * slot_bytes;
+    const int stage_bytes = hdr_bytes + CH * slot_bytes;
     unsigned char* stages = smem + stages_off;
 
     if (tid == 0) {
@@ -268,59 +268,53 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     __syncthreads();
 
     const int nch = c_end - c_begin;
-    const int nstage = (nch + kWinCh - 1) / kWinCh;
+    const int nstage = (nch + CH - 1) / CH;
     const int stage_total = a.stage_total;
 
     if (warp >= NCW) {
-        // ---- producer warp group: gives its registers to the consumers; one thread stages kWinCh
+        // ---- producer warp group: gives its registers to the consumers; one thread stages CH
         // channels per barrier (padding channels and the extra last stage get zeros)
         asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
         {
-            // the four warps of the group take the stages in turn (stage s belongs to warp s % 4), so
-            // the staging work is spread over the four schedulers instead of loading the one that also
-            // runs consumer warps 0, 4, 8
+            // the warps of the group take the stages in turn (stage s belongs to warp s % P), so the staging
+            // work is spread over the schedulers instead of loading the one that also runs consumer warps
+            // 0, 4, 8.  P = min(4, nst): a warp waits on a slot's empty barrier by parity only, it is ordered
+            // behind stage s - P - nst, and the parity test needs stage s - 2 * nst consumed (P <= nst).
             const int pw = warp - NCW;
+            const int P = nst < 4 ? nst : 4;
             const int32_t* meta = a.meta + (static_cast<int64_t>(ty) * a.nchans + c_begin) * kWinMetaWords;
-            const int32_t* hdr = a.hdr + (static_cast<int64_t>(ty) * stage_total + stage0) * kWinHdrWords;
+            const int32_t* hdr = a.hdr + (static_cast<int64_t>(ty) * stage_total + stage0) * a.hdr_words;
             const float2* prow = static_cast<const float2*>(a.pairs) +
                                  (static_cast<int64_t>(beam) * a.nchans + c_begin) * a.pair_stride + T0;
             const int64_t pair_stride = a.pair_stride;
             const int zlen = ((NT - 1) * W + W + 2 + 1) & ~1;  // pairs a padding channel must provide
-            for (int s = pw; s < nstage; s += 4) {
+            for (int s = pw; s < nstage && pw < P; s += P) {
                 const int ring = s % nst, lap = s / nst;
-                // lanes 0 .. kWinCh-1: (base, len) of this stage's channels
-                const int k = s * kWinCh + lane;
+                // lanes 0 .. CH-1: (base, len) of this stage's channels
+                const int k = s * CH + lane;
                 int pb = 0, pl = -1;
-                if (lane < kWinCh && k < nch) {
+                if (lane < CH && k < nch) {
                     pb = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords);
                     pl = __ldg(meta + static_cast<int64_t>(k) * kWinMetaWords + 1);
                 }
-                int base[kWinCh], len[kWinCh];
+                unsigned bytes = lane < CH ? (pl < 0 ? zlen : pl) * 8 : 0;
 #pragma unroll
-                for (int ch = 0; ch < kWinCh; ++ch) {
-                    base[ch] = __shfl_sync(0xffffffffu, pb, ch);
-                    len[ch] = __shfl_sync(0xffffffffu, pl, ch);
-                }
+                for (int o = 8; o > 0; o >>= 1)   // CH <= 12 < 16 lanes
+                    bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
                 if (lane == 0) {
                     if (lap > 0)
                         mbar_wait_backoff(bar_empty + 8u * ring, (lap - 1) & 1);
-                    const unsigned dst = smem_u32(stages) + ring * stage_bytes;
-                    const unsigned fb = bar_full + 8u * ring;
-                    unsigned bytes = kWinHdrWords * 4;
-#pragma unroll
-                    for (int ch = 0; ch < kWinCh; ++ch)
-                        bytes += (len[ch] < 0 ? zlen : len[ch]) * 8;
-                    mbar_expect_tx(fb, bytes);
-                    bulk_g2s(dst, hdr + static_cast<int64_t>(s) * kWinHdrWords, kWinHdrWords * 4, fb);
-#pragma unroll
-                    for (int ch = 0; ch < kWinCh; ++ch) {
-                        const unsigned d = dst + kWinHdrWords * 4 + ch * slot_bytes;
-                        if (len[ch] < 0)
-                            bulk_g2s(d, a.zeros, zlen * 8, fb);
-                        else
-                            bulk_g2s(d, prow + static_cast<int64_t>(s * kWinCh + ch) * pair_stride + base[ch],
-                                     len[ch] * 8, fb);
-                    }
+                    mbar_expect_tx(bar_full + 8u * ring, bytes + hdr_bytes);
+                    bulk_g2s(smem_u32(stages) + ring * stage_bytes, hdr + static_cast<int64_t>(s) * a.hdr_words, hdr_bytes,
+                             bar_full + 8u * ring);
+                }
+                __syncwarp();   // the expected byte count is posted before any lane's copy can complete
+                if (lane < CH) {
+                    const unsigned d = smem_u32(stages) + ring * stage_bytes + hdr_bytes + lane * slot_bytes;
+                    if (pl < 0)
+                        bulk_g2s(d, a.zeros, zlen * 8, bar_full + 8u * ring);
+                    else
+                        bulk_g2s(d, prow + static_cast<int64_t>(k) * pair_stride + pb, pl * 8, bar_full + 8u * ring);
                 }
                 __syncwarp();
             }
@@ -368,7 +362,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // per stage: wait for the NEXT stage and read its four metadata words with one LDS.128, then
     // add the four channels of this stage; the window of channel k+1 is loaded while channel k is
     // added (wa / wb alternate).
-    const unsigned lane_off = kWinHdrWords * 4 + (wt * W + lane_pinned * T) * 8;  // bytes from the slot start
+    const unsigned lane_off = hdr_bytes + (wt * W + lane_pinned * T) * 8;  // bytes from the stage start
     auto shifts = [&](unsigned m) {
         const unsigned sm = (m >> 5) & 0x3ffu;
         shift_rows<T, D, OutT>(acc, sm & 31u, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
@@ -382,7 +376,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // and a stage boundary is nothing but the barrier traffic (arrive, wait for the next stage).  Every
     // uniform-datapath instruction in the per-channel chain costs its full latency with three warps per
     // scheduler, so that chain is kept to the window address.
-    const unsigned hdr_off = 4 * kWinCh * g;
+    const unsigned hdr_off = 4 * CH * g;
     unsigned m = __ldg(a.first + (static_cast<int64_t>(ty) * a.nband + band) * G + g);
     m = __reduce_or_sync(0xffffffffu, m);   // warp-uniform by construction; this lets ptxas know
     mbar_wait(bar_full, 0);
@@ -402,7 +396,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             // threaded code (window_rows.inc, chan_loop): one indirect branch per channel over the 8 offset
             // patterns; runs channels until the stage is done or one needs a row shift
             unsigned spa = smem_u32(sbase) + lane_off;  // this thread's window base in the stage's first slot
-            unsigned chn = kWinCh;
+            unsigned chn = CH;
             while (true) {
                 chan_loop(acc, m, hw, spa, chn, static_cast<unsigned>(slot_bytes));
                 if (chn == 0)
@@ -418,7 +412,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             if (m & kWinStageShift) {
                 // a row shift somewhere in this stage (about a third of the stages)
 #pragma unroll 1
-                for (int ch = 0; ch < kWinCh; ++ch) {
+                for (int ch = 0; ch < CH; ++ch) {
                     const unsigned mn = lds32(hw);
                     load_window<T>(w, sp + (m >> 21) * 8);
                     if (m & kWinShiftBits)
@@ -430,7 +424,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
                 }
             } else {
 #pragma unroll 1
-                for (int ch = 0; ch < kWinCh; ++ch) {
+                for (int ch = 0; ch < CH; ++ch) {
                     const unsigned mn = lds32(hw);
                     load_window<T>(w, sp + (m >> 21) * 8);
                     rows7(acc, w, m);
@@ -599,40 +593,16 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
 // ------------------------------------------------------------------------------------------------
 // launcher
 // ------------------------------------------------------------------------------------------------
-// number of pipeline stages that fit into shared memory (0: the kernel cannot run)
-static int window_ring(const WindowGeom& g, int lmax, int* slot_bytes)
-{
-    const int sb = (lmax * 8 + 127) & ~127;
-    const int fixed = kWinFixedBytes;  // barriers, hand-over state; the transpose scratch aliases the ring
-    const int budget = (g.G * g.NT == 4 ? 113 : 227) * 1024 - fixed;
-    const int stage_bytes = kWinHdrWords * 4 + kWinCh * sb;
-    int nst = budget / stage_bytes;
-    if (nst > 8)
-        nst = 8;
-    *slot_bytes = sb;
-    if (nst * stage_bytes < g.G * g.NT * g.W() * 8)
-        return 0;
-    // Four producer warps take the stages in turn and wait on a slot's empty barrier by parity only: a
-    // warp is ordered behind stage s - 4 - nst, the parity test needs stage s - 2 * nst consumed, which
-    // holds from four stages on.
-    return nst >= 4 ? nst : 0;
-}
-
-bool window_fits_smem(const WindowPlan& wp)
-{
-    int sb;
-    return wp.ok && window_ring(wp.geom, wp.lmax, &sb) > 0;
-}
+bool window_fits_smem(const WindowPlan& wp) { return wp.ok && wp.nst >= 2; }
 
 template <int T, int G, int NT, int D, typename OutT>
 static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
 {
-    int slot_bytes = 0;
-    const int nst = window_ring(a.geom, a.lmax, &slot_bytes);
-    if (nst == 0)
+    const int nst = a.nst, slot_bytes = a.slot_bytes;
+    if (nst < 2)
         return static_cast<int>(cudaErrorInvalidConfiguration);
     const int stages_off = kWinFixedBytes;
-    const size_t ring = static_cast<size_t>(nst) * (kWinHdrWords * 4 + kWinCh * slot_bytes);
+    const size_t ring = static_cast<size_t>(nst) * (a.hdr_words * 4 + a.ch * slot_bytes);
     const size_t smem = static_cast<size_t>(stages_off) + ring;
     WindowArgs a2 = a;  // rows per flush pass: as many [NCW][W] u64 transposes as the ring holds
     a2.flush_rows = static_cast<int>(ring / (static_cast<size_t>(G) * NT * 32 * T * 8));
@@ -643,8 +613,7 @@ static int launch_bands(const WindowArgs& a, cudaStream_t st, int* launches)
         return static_cast<int>(e);
     dim3 grid(static_cast<unsigned>(a.ntile_dm) * a.ntile_t, 1, a.nbeams);
     for (int b = 0; b < a.nband; ++b) {
-        window_kernel<T, G, NT, D, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a2, a.band[b], a.band[b + 1], b,
-                                                                              a.stage0[b], nst, slot_bytes);
+        window_kernel<T, G, NT, D, OutT><<<grid, (G * NT + 4) * 32, smem, st>>>(a2, a.band[b], a.band[b + 1], b, a.stage0[b]);
         ++*launches;
         e = cudaGetLastError();
         if (e != cudaSuccess)

@@ -221,18 +221,56 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
             }
         }
     }
-    // ---- stage headers: the kernel consumes kWinCh channels per barrier.  A consumer warp carries the
+    // ---- ring of staged segments.  Stage boundaries cost every consumer warp an arrive, a barrier wait
+    // and a refill of its pipeline (11.5 % of the kernel with 4-channel stages), so stages should be long;
+    // the ring must still hold >= 2 of them.  Measured on cfg 3 (slots of 9.3 / 12.5 KB): 8 channels x 3
+    // stages beat 12 x 2, 6 x 4 and 4 x 6; 9 x 2 beats 6 x 3.  Rule: the longest stage <= 12 channels that
+    // leaves three stages if that is >= 8 channels, else the longest that leaves two.
+    {
+        const int sb = (lmax * 8 + 127) & ~127;
+        const int budget = (G * geom.NT == 4 ? 113 : 227) * 1024 - kWinFixedBytes;
+        auto stage_bytes = [&](int ch) { return (G * ch * 4 + 127) / 128 * 128 + ch * sb; };
+        auto longest = [&](int nst) {
+            int ch = 0;
+            for (int c = 1; c <= kWinChMax; ++c)
+                if (nst * stage_bytes(c) <= budget)
+                    ch = c;
+            return ch;
+        };
+        int ch = longest(3), nstg = 3;
+        if (ch < 8) {
+            const int c2 = longest(2);
+            if (c2 > ch) {
+                ch = c2;
+                nstg = 2;
+            }
+        }
+        wp.lmax = lmax;
+        wp.slot_bytes = sb;
+        // the flush's transpose scratch ([warps][W] pairs per row) overlays the ring
+        if (ch < 2 || nstg * stage_bytes(ch) < G * geom.NT * W * 8) {
+            wp.ch = wp.nst = wp.hdr_words = 0;  // does not fit shared memory: ok stays false
+            return false;
+        }
+        while ((nstg + 1) * stage_bytes(ch) <= budget && nstg < 8)
+            ++nstg;
+        wp.ch = ch;
+        wp.nst = nstg;
+        wp.hdr_words = (G * ch * 4 + 127) / 128 * 32;
+    }
+    const int CH = wp.ch, HW = wp.hdr_words;
+    // ---- stage headers.  A consumer warp carries the
     // current channel's word in a (uniform) register and reads the NEXT channel's word while it adds, so
-    // the header of a stage holds, regrouped per row group (hdr[g * kWinCh + ch]), the words of the
+    // the header of a stage holds, regrouped per row group (hdr[g * CH + c]), the words of the
     // channels one further on; the band's first word comes from `first`.  The word of a channel that
     // opens a stage says whether any channel of that stage has a row shift (the kernel then runs the
     // loop variant that tests for shifts).  Channels past the band's end and one extra stage per band
     // stay zero (the kernel stages a zero segment for them).
     wp.stage0.assign(wp.nband + 1, 0);
     for (int b = 0; b < wp.nband; ++b)
-        wp.stage0[b + 1] = wp.stage0[b] + (wp.band[b + 1] - wp.band[b] + kWinCh - 1) / kWinCh + 1;
+        wp.stage0[b + 1] = wp.stage0[b] + (wp.band[b + 1] - wp.band[b] + CH - 1) / CH + 1;
     const int nst = wp.stage0[wp.nband];
-    wp.hdr.assign(static_cast<size_t>(ntile) * nst * kWinHdrWords, 0);
+    wp.hdr.assign(static_cast<size_t>(ntile) * nst * HW, 0);
     wp.first.assign(static_cast<size_t>(ntile) * wp.nband * G, 0);
     for (int ty = 0; ty < ntile; ++ty)
         for (int b = 0; b < wp.nband; ++b) {
@@ -241,22 +279,20 @@ bool build_window_plan(const int32_t* shift, int ndm, int nchans, const WindowGe
                 auto word_of = [&](int c) -> uint32_t& {
                     return reinterpret_cast<uint32_t&>(wp.meta[(static_cast<size_t>(ty) * nchans + c) * kWinMetaWords + 2 + g]);
                 };
-                for (int cs = c0; cs < c1; cs += kWinCh) {
+                for (int cs = c0; cs < c1; cs += CH) {
                     bool any = false;
-                    for (int c = cs; c < std::min(cs + kWinCh, c1); ++c)
+                    for (int c = cs; c < std::min(cs + CH, c1); ++c)
                         any = any || (word_of(c) & kWinShiftBits) != 0;
                     if (any)
                         word_of(cs) |= kWinStageShift;
                 }
                 wp.first[(static_cast<size_t>(ty) * wp.nband + b) * G + g] = static_cast<int32_t>(word_of(c0));
                 for (int c = c0; c + 1 < c1; ++c) {
-                    const int s = wp.stage0[b] + (c - c0) / kWinCh, ch = (c - c0) % kWinCh;
-                    wp.hdr[(static_cast<size_t>(ty) * nst + s) * kWinHdrWords + g * kWinCh + ch] =
-                        static_cast<int32_t>(word_of(c + 1));
+                    const int s = wp.stage0[b] + (c - c0) / CH, cc = (c - c0) % CH;
+                    wp.hdr[(static_cast<size_t>(ty) * nst + s) * HW + g * CH + cc] = static_cast<int32_t>(word_of(c + 1));
                 }
             }
         }
-    wp.lmax = lmax;
     wp.maxbase = maxbase;
     wp.theta_max = theta_max;
     wp.ok = true;

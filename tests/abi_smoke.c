@@ -19,7 +19,7 @@ int main(void)
     dedisp_stream *stream = NULL;
     dedisp_survey *survey = NULL;
     dedisp_pass pass = {0.0, 0.1, 24, 12, 2};
-    int64_t info[12], total = 0;
+    int64_t info[14], total = 0;
     int d, c;
 
     for (d = 0; d < NDM; ++d)
