@@ -87,7 +87,7 @@ def chan_loop(T, D):
         # loads and row 0 of the channel whose word is m; exits first if it needs a row shift
         X = ["and.b32 t, %%%d, %d; setp.ne.u32 ps, t, 0; @ps bra.uni DONE_%%=;" % (M, 0x7fe0)]
         X.append("ld.shared.u32 mn, [%%%d];" % HW)
-        X.append("shr.u32 t, %%%d, 21; shl.b32 t, t, 3; add.u32 a, %%%d, t;" % (M, SP))
+        X.append("shr.u32 t, %%%d, 18; and.b32 t, t, 0x3ff8; add.u32 a, %%%d, t;" % (M, SP))
         X += ["ld.shared.b64 w%d, [a+%d];" % (k, 8 * k) for k in range(T + 1)]
         X.append("and.b32 idx, %%%d, %d;" % (M, NP - 1))
         X += adds(0, 0)
