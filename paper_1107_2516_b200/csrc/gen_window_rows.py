@@ -133,7 +133,7 @@ def main():
     out = ["// GENERATED by gen_window_rows.py -- do not edit.\n"]
     for D, T in COMBOS:
         out.append(rows7(T, D))
-        if D == 4:  # 8 variants; with 5 rows (16) it is no faster than the chains, with 6 (32) far slower (I-cache)
+        if D == 4 or (D == 5 and T <= 11):  # 8 variants; 16 pay while their code stays small (5 x 11: 48.6 -> 44.4 ms); with 5 rows (16) it is no faster than the chains, with 6 (32) far slower (I-cache)
             out.append(chan_loop(T, D))
     for T in sorted({t for _, t in COMBOS}):
         out.append(shift_row(T))

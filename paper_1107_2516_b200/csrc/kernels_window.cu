@@ -392,7 +392,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             par_n ^= 1u;
         }
         unsigned hw = smem_u32(sbase) + hdr_off;    // this row group's words of the channels one further on
-        if constexpr (D == 4) {
+        if constexpr (D == 4 || (D == 5 && T <= 11)) {
             // threaded code (window_rows.inc, chan_loop): one indirect branch per channel over the 8 offset
             // patterns; runs channels until the stage is done or one needs a row shift
             unsigned spa = smem_u32(sbase) + lane_off;  // this thread's window base in the stage's first slot
