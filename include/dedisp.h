@@ -58,7 +58,7 @@ typedef enum {
     DEDISP_ENOMEM = 2, /* host or device allocation failed                                */
     DEDISP_ECUDA = 3,  /* CUDA runtime error (no device, launch failure, ...)             */
     DEDISP_ESHAPE = 4, /* strides / lengths inconsistent with the plan                    */
-    DEDISP_ESTATE = 5  /* call not valid for this kind of plan or stream                  */
+    DEDISP_ESTATE = 5  /* call not valid for this plan / stream, or no covering reservation   */
 } dedisp_status;
 
 typedef enum {
@@ -67,11 +67,12 @@ typedef enum {
 } dedisp_dtype;
 
 /* Kernel choice for dedisp_plan_set_kernel.  AUTO picks, for brute-force plans, the register-window
- * kernel when the plan's shift table fits its limits; otherwise, and for both stages of subband
- * plans, the long-tile kernel (rows of >= 4096 samples) or the direct kernel (shorter rows). */
+ * kernel when the plan's shift table fits its limits and the problem fills the device (see
+ * dedisp_plan_resolved_kernel); otherwise, and for both stages of subband plans, the long-tile kernel
+ * (rows of >= 4096 samples) or the direct kernel (shorter rows). */
 typedef enum {
     DEDISP_KERNEL_AUTO = 0,
-    DEDISP_KERNEL_NAIVE = 1,  /* one thread per output sample, global loads only (debug)    */
+    DEDISP_KERNEL_NAIVE = 1,  /* one thread per output sample, global loads only (AUTO's choice for tiny problems) */
     DEDISP_KERNEL_DIRECT = 2, /* shared-memory staged, register-blocked DMs x time           */
     DEDISP_KERNEL_WINDOW = 3, /* + one register window shared by the DM rows of a thread     */
     DEDISP_KERNEL_LONG = 4    /* 16 rows x 2048 samples per block, TMA-staged channel unions  */
