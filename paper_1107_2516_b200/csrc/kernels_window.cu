@@ -364,10 +364,14 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     // added (wa / wb alternate).
     const unsigned lane_off = hdr_bytes + (wt * W + lane_pinned * T) * 8;  // bytes from the stage start
     auto shifts = [&](unsigned m) {
-        const unsigned sm = (m >> 5) & 0x3ffu;
-        shift_rows<T, D, OutT>(acc, sm & 31u, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
-        if (sm >> 5)
-            shift_rows<T, D, OutT>(acc, sm >> 5, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
+        // two masks (a row may shift twice at one channel); ONE copy of the shift code: it runs at 2 % of
+        // the channels and its instruction fetches miss
+        unsigned sm = (m >> 5) & 0x3ffu;
+#pragma unroll 1
+        do {
+            shift_rows<T, D, OutT>(acc, sm & 31u, lane_pinned, fall_s, static_cast<unsigned>(a.n_out), hp, wt < NT - 1, first, edge);
+            sm >>= 5;
+        } while (sm);
     };
     // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
     // accumulator registers between copies otherwise).  A warp carries the current channel's word m in a
