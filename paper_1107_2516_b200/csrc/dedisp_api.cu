@@ -102,9 +102,10 @@ struct dedisp_plan {
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};  // start, end, between the subband stages
     bool ev_valid = false, ev_mid_valid = false;
     // dedisp_execute_host pipeline: copy streams and per-chunk events (created on first use)
-    static constexpr int kHostChunks = 8;
+    static constexpr int kHostChunks = 8;   // time pieces of the host entries (+ 1: the first is split)
+    static constexpr int kHostEvents = kHostChunks + 2;
     cudaStream_t copy_st[2] = {nullptr, nullptr};  // H2D, D2H
-    cudaEvent_t ev_copy[2 * kHostChunks + 2] = {};
+    cudaEvent_t ev_copy[2 * kHostEvents + 2] = {};
 };
 
 struct dedisp_stream {
@@ -490,6 +491,21 @@ dedisp_status reserve(dedisp_plan* plan, dedisp_dtype dtype, int64_t nsamp_out, 
     return DEDISP_OK;
 }
 
+// Time piece i of a host-entry execute: uniform pieces of csize samples, the first one split at a quarter so
+// that the first kernel (and with it the first device-to-host copy) starts after a quarter of the wait.
+// Returns false past the end.
+bool host_piece(int64_t nsamp, int64_t csize, int i, int64_t* t0, int64_t* cn)
+{
+    const int64_t q = round_up(csize / 4, 64);
+    const int64_t b0 = i == 0 ? 0 : i == 1 ? q : static_cast<int64_t>(i - 1) * csize;
+    const int64_t b1 = i == 0 ? q : static_cast<int64_t>(i) * csize;
+    if (b0 >= nsamp)
+        return false;
+    *t0 = b0;
+    *cn = (b1 < nsamp ? b1 : nsamp) - b0;
+    return true;
+}
+
 bool ensure_copy_streams(dedisp_plan* plan)
 {
     if (plan->copy_st[0])
@@ -830,9 +846,9 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
         return DEDISP_ECUDA;
     cudaStream_t h2d = plan->copy_st[0], d2h = plan->copy_st[1];
     cudaEvent_t* ev_in = plan->ev_copy;                              // [nchunk] input columns landed
-    cudaEvent_t* ev_ex = plan->ev_copy + dedisp_plan::kHostChunks;   // [nchunk] kernels of the chunk done
-    cudaEvent_t ev_start = plan->ev_copy[2 * dedisp_plan::kHostChunks];
-    cudaEvent_t ev_done = plan->ev_copy[2 * dedisp_plan::kHostChunks + 1];
+    cudaEvent_t* ev_ex = plan->ev_copy + dedisp_plan::kHostEvents;   // [nchunk] kernels of the chunk done
+    cudaEvent_t ev_start = plan->ev_copy[2 * dedisp_plan::kHostEvents];
+    cudaEvent_t ev_done = plan->ev_copy[2 * dedisp_plan::kHostEvents + 1];
     const int64_t csize = round_up((nsamp_out + nchunk - 1) / nchunk, 64);
     bool ok = cudaEventRecord(ev_start, st) == cudaSuccess &&
               cudaStreamWaitEvent(h2d, ev_start, 0) == cudaSuccess &&
@@ -843,11 +859,10 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
     char* hout = static_cast<char*>(host_out);
     int launches = 0;
     int64_t col = 0;  // input columns copied so far
-    for (int i = 0; i < nchunk && ok; ++i) {
-        const int64_t t0 = i * csize;
-        if (t0 >= nsamp_out)
+    for (int i = 0; i <= nchunk && ok; ++i) {
+        int64_t t0, cn;
+        if (!host_piece(nsamp_out, csize, i, &t0, &cn))
             break;
-        const int64_t cn = nsamp_out - t0 < csize ? nsamp_out - t0 : csize;
         const int64_t need = t0 + cn + plan->max_delay;  // input columns chunk i reads
         if (need > col) {
             ok = cudaMemcpy2DAsync(din + col * es, in_stride * es, hin + col * es, n_in * es, (need - col) * es,
@@ -998,9 +1013,9 @@ dedisp_status dedisp_stream_push_host(dedisp_stream* s, const void* host_chunk_i
     char* hout = static_cast<char*>(host_out);
     cudaStream_t h2d = p->copy_st[0], d2h = p->copy_st[1];
     cudaEvent_t* ev_in = p->ev_copy;
-    cudaEvent_t* ev_ex = p->ev_copy + dedisp_plan::kHostChunks;
-    cudaEvent_t ev_start = p->ev_copy[2 * dedisp_plan::kHostChunks];
-    cudaEvent_t ev_done = p->ev_copy[2 * dedisp_plan::kHostChunks + 1];
+    cudaEvent_t* ev_ex = p->ev_copy + dedisp_plan::kHostEvents;
+    cudaEvent_t ev_start = p->ev_copy[2 * dedisp_plan::kHostEvents];
+    cudaEvent_t ev_done = p->ev_copy[2 * dedisp_plan::kHostEvents + 1];
     bool ok = cudaEventRecord(ev_start, st) == cudaSuccess && cudaStreamWaitEvent(h2d, ev_start, 0) == cudaSuccess &&
               cudaStreamWaitEvent(d2h, ev_start, 0) == cudaSuccess;
     int launches = 0;
@@ -1162,8 +1177,9 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
     const bool fused = fused_stats_ok(plan, dtype, csize);
     int64_t npart_total = 0;
     if (fused) {
-        for (int64_t t0 = 0; t0 < nsamp_out; t0 += csize)
-            npart_total += static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, std::min(csize, nsamp_out - t0));
+        int64_t t0, cn;
+        for (int i = 0; (nchunk == 1 ? i == 0 : host_piece(nsamp_out, csize, i, &t0, &cn)); ++i)
+            npart_total += static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nchunk == 1 ? nsamp_out : cn);
         if (plan->det_partial.ensure(static_cast<size_t>(nbeams) * npart_total * 2 * sizeof(double)) != cudaSuccess) {
             cudaGetLastError();
             return DEDISP_ENOMEM;
@@ -1173,7 +1189,7 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
         return DEDISP_ECUDA;
     cudaStream_t h2d = plan->copy_st[0];
     cudaEvent_t* ev_in = plan->ev_copy;
-    cudaEvent_t ev_start = plan->ev_copy[2 * dedisp_plan::kHostChunks];
+    cudaEvent_t ev_start = plan->ev_copy[2 * dedisp_plan::kHostEvents];
     bool ok = cudaEventRecord(ev_start, st) == cudaSuccess && cudaStreamWaitEvent(h2d, ev_start, 0) == cudaSuccess;
     const char* hin = static_cast<const char*>(host_in);
     char* din = static_cast<char*>(plan->host_in.p);
@@ -1182,11 +1198,10 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
     const Elem in_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::U8;
     int launches = 0;
     int64_t col = 0, part_off = 0;
-    for (int i = 0; i < nchunk && ok; ++i) {
-        const int64_t t0 = i * csize;
-        if (t0 >= nsamp_out)
+    for (int i = 0; i <= nchunk && ok; ++i) {
+        int64_t t0 = 0, cn = nsamp_out;
+        if (nchunk == 1 ? i > 0 : !host_piece(nsamp_out, csize, i, &t0, &cn))
             break;
-        const int64_t cn = std::min(csize, nsamp_out - t0);
         const int64_t need = t0 + cn + plan->max_delay;
         if (need > col) {
             ok = cudaMemcpy2DAsync(din + col * es, in_stride * es, hin + col * es, n_in * es, (need - col) * es, rows_in,
