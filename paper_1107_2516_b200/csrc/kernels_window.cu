@@ -7,20 +7,23 @@
 //     fp32 here; sums of < 2^24/255 bytes are exact in fp32).  Two samples NT*W apart that share
 //     (c, d) have the same shift, so the main kernel adds two outputs per instruction
 //     (add.f32x2 -> FADD2) from naturally aligned 64-bit registers, whatever the shift's parity.
-//  2. window_kernel (band b): a block = G row groups x NT warps; a consumer
-//     warp owns 8 DM rows x 32*T slots (pairs of output samples) and keeps their 8 x T packed
-//     accumulators in registers for the whole band.  Per channel it loads ONE window of T + 1
-//     staged pairs (LDS.64, conflict-free for odd T) that feeds all 8 rows: row j adds
-//     w[i + o_j], o_j in {0, 1} chosen by a warp-uniform two-way branch (window_rows.inc).  Rows
-//     follow the growing delay difference between neighbouring DM trials by moving their
-//     accumulators up one slot now and then ("row shift", planned on the host: window_plan.cpp);
-//     the partial sum that leaves the top of the warp's slot range is handed, through the output
-//     buffer, to the warp segment that follows in time (its fresh bottom slot stands for the same
-//     output sample), so a block of 2*NT segments loses kmax samples as a whole, not per segment.
-//     Channel segments are staged into a ring of shared-memory slots by 1-D TMA bulk copies
-//     (cp.async.bulk + mbarrier) issued by thread 0 a few channels ahead.  At the end of the band the
-//     accumulators go through a per-warp shared-memory transpose to coalesced global accesses:
-//     band 0 stores, later bands add to what is there.
+//  2. window_kernel (band b): a block = G row groups x NT warps along time (+ a producer warp
+//     group); a consumer warp owns D DM rows x 32*T slots (pairs of output samples) and keeps their
+//     D x T packed accumulators in registers for the whole band.  Per channel it loads ONE window of
+//     T + 1 staged pairs (LDS.64, conflict-free for odd T) that feeds all D rows: row j adds
+//     w[i + o_j], o_j in {0, 1}, a warp-uniform choice per row and channel.  4-row shapes run the
+//     channels of a pipeline stage as threaded code (chan_loop in window_rows.inc: one indirect
+//     branch per channel over the 2^(D-1) offset patterns), 6-row shapes as two chains of row blocks
+//     (rows7: one uniform branch per change of offset).  Rows follow the growing delay difference
+//     between neighbouring DM trials by moving their accumulators up one slot now and then ("row
+//     shift", planned on the host: window_plan.cpp); the partial sum that leaves the top of the
+//     warp's slot range is handed, through the output buffer, to the warp segment that follows in
+//     time (its fresh bottom slot stands for the same output sample), so a block of 2*NT segments
+//     loses kmax samples as a whole, not per segment.  Channel segments are staged into a ring of
+//     2-3 pipeline stages of 8-12 channels by 1-D TMA bulk copies (cp.async.bulk + mbarrier), every
+//     lane of a producer warp issuing one channel's copy.  At the end of the band the accumulators go
+//     through a per-warp shared-memory transpose to coalesced global accesses: band 0 stores (and,
+//     for dedisp_execute_detect, sums the outputs' statistics), later bands add to what is there.
 #include <cuda_runtime.h>
 
 #include "dedisp_internal.h"
@@ -359,9 +362,6 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     }
     __syncwarp();
 
-    // per stage: wait for the NEXT stage and read its four metadata words with one LDS.128, then
-    // add the four channels of this stage; the window of channel k+1 is loaded while channel k is
-    // added (wa / wb alternate).
     const unsigned lane_off = hdr_bytes + (wt * W + lane_pinned * T) * 8;  // bytes from the stage start
     auto shifts = [&](unsigned m) {
         // two masks (a row may shift twice at one channel); ONE copy of the shift code: it runs at 2 % of
@@ -373,8 +373,9 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
             sm >>= 5;
         } while (sm);
     };
-    // Stage loop around a channel loop with a single copy of the add block (ptxas permutes the
-    // accumulator registers between copies otherwise).  A warp carries the current channel's word m in a
+    // Stage loop around the channels of a stage.  (Sequential C++ copies of the add block make ptxas
+    // permute the accumulator registers between them -- hundreds of moves -- so the chains keep ONE copy
+    // in a rolled loop and the threaded loop is a single PTX statement.)  A warp carries the current channel's word m in a
     // uniform register; the NEXT channel's word is read from the stage's header at the top of the
     // iteration, next to the window loads, and moved into m after the adds, so its latency never shows
     // and a stage boundary is nothing but the barrier traffic (arrive, wait for the next stage).  Every
