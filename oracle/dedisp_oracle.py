@@ -10,8 +10,10 @@ arrays into it, and adds ``brute_samples`` -- the definition written out with nu
 single output samples (used to spot-check full-size GPU runs).
 
 Pins: see the header of ``dedisp_oracle.c`` and ``tests/test_oracle_pins.py``.  ``brute_samples``
-is pinned by equality with ``brute_f32`` / ``brute_u8`` on the pinned small cases.  The absolute
-sensitivity loss of the subband method is "parity unpinned".
+is pinned by equality with ``brute_f32`` / ``brute_u8`` on the pinned small cases; ``survey`` (the
+multi-pass plan of PAPER.md Tables 1 / 4: binning -> stage 1 -> stage 2 per pass) has no arithmetic of
+its own and is pinned by the single-pass identity, Table 4's counts (tests/golden/table4_plan.txt) and
+pulse recovery in every pass.  The absolute sensitivity loss of the subband method is "parity unpinned".
 """
 import ctypes
 import os
