@@ -241,7 +241,7 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     constexpr int kPool = ((NCW == 4 ? 32768 : 65536) - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
     constexpr int kConsRegs = kPool > 240 ? 240 : kPool;
     static_assert(NCW % 4 == 0, "setmaxnreg works on groups of four warps");
-    static_assert(NCW <= 16 && D <= kWinD, "Fall area");
+    static_assert(NCW <= 12 && D <= kWinD, "hand-over area; shapes with 16 consumer warps (120 registers each) hung in a trial and are not supported");
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // Block order: groups of a.dm_group DM tiles; inside a group all time tiles, DM tile fastest.
