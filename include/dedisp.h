@@ -29,8 +29,9 @@
  *     of plan, and calls on one plan must not be made from several threads at once.  Use one
  *     plan per CUDA stream for concurrent work.  A plan lives on the device that was current at
  *     its first dedisp_plan_reserve.
- *   - No exceptions cross this boundary, nothing calls exit(), there is no global state and the
- *     library reads no environment variables.
+ *   - No exceptions cross this boundary, nothing calls exit(), the library reads no environment
+ *     variables and keeps no global state -- with one exception, the fixed device array behind
+ *     dedisp_detect_static (described there).
  *   - There is no CPU fallback: without a CUDA device every execute/push returns DEDISP_ECUDA.
  *     Plan creation and the table getters are host-only and work without a device.
  */
@@ -58,7 +59,8 @@ typedef enum {
     DEDISP_ENOMEM = 2, /* host or device allocation failed                                */
     DEDISP_ECUDA = 3,  /* CUDA runtime error (no device, launch failure, ...)             */
     DEDISP_ESHAPE = 4, /* strides / lengths inconsistent with the plan                    */
-    DEDISP_ESTATE = 5  /* call not valid for this plan / stream, or no covering reservation   */
+    DEDISP_ESTATE = 5, /* call not valid for this plan / stream, or no covering reservation   */
+    DEDISP_ELIMIT = 6  /* larger than the fixed scratch of an allocation-free entry point     */
 } dedisp_status;
 
 typedef enum {
@@ -292,6 +294,56 @@ DEDISP_API dedisp_status dedisp_plan_detect(dedisp_plan *plan, const void *out, 
  * pivot = sum_c in[c][0], reduced in a fixed order), so detection costs ONE pass over the buffer (the
  * threshold scan) instead of two; other plans run dedisp_execute followed by dedisp_plan_detect.  Same
  * definition of mean / sigma / threshold / events either way.  Asynchronous; needs dedisp_plan_reserve.
+/*
+ * dedisp_detect_static -- the event detection of dedisp_plan_detect (PAPER.md:76; same kernels, same
+ * definition of mean / sigma / threshold / events, same summation order, hence the same numbers) for
+ * callers that cannot let the library allocate device memory.
+ *
+ * Who that is.  dedisp_plan_detect keeps its per-block partial sums in a workspace that
+ * dedisp_plan_reserve obtains with cudaMalloc.  Two kinds of user cannot afford that call:
+ *   - the processing thread of a real-time backend (the paper's pipeline, PAPER.md:281-285): cudaMalloc
+ *     and cudaFree serialise on a driver lock, and replacing a workspace by a larger one frees the old
+ *     one, which waits for the whole device to go idle -- the copy stream that is receiving the next
+ *     buffer from the telescope included -- so a reservation that grows in the middle of an observation
+ *     costs samples;
+ *   - a host application that claimed the whole of the GPU's memory for its own ring buffers or pool
+ *     when it started: whatever the library asks the driver for afterwards simply fails.
+ * This entry needs no plan and no reserve.  Its only scratch is an array of
+ * DEDISP_DETECT_STATIC_MAX_SLOTS x 16 bytes (296 KiB) that is compiled into the library: every GPU on
+ * which the process uses the library holds one copy from the moment the module is loaded until the
+ * process ends, whether or not this function is ever called.  The caller supplies everything else.
+ *
+ *   out, dtype, nsamp_out, out_stride, nbeams, nsigma, events, capacity, results
+ *              exactly as for dedisp_plan_detect (all DEVICE pointers, caller-owned)
+ *   ndm        DM trials (rows) per beam in `out` (> 0); the plan is not needed for anything else
+ *
+ * Limit: nbeams * min(ndm, 1184) <= DEDISP_DETECT_STATIC_MAX_SLOTS (18944: e.g. 16 beams of any number
+ * of trials, or 74 beams of 256 trials).  Anything larger returns DEDISP_ELIMIT before the device is
+ * touched; the array is never enlarged.  dedisp_detect_static_max_slots() returns the same constant for
+ * callers that do not compile against this header.
+ *
+ * First call on a device: the library asks the runtime for the device address of the array
+ * (cudaGetSymbolAddress, under a mutex, result cached per device).  That look-up may make the runtime
+ * load the library's device code, so make the first call on each GPU during start-up, with that GPU
+ * current, and before any stream capture is begun.  Later calls only launch three kernels on
+ * cuda_stream; no call ever runs cudaMalloc, cudaFree or an allocating library routine, and none
+ * synchronises.
+ *
+ * Sharing: all calls on one GPU, from every thread and stream, use the same array, and it keeps
+ * whatever the previous call wrote.  Nothing in it needs to be zero on entry -- a call overwrites every
+ * slot before it reads it -- but two calls that run on the GPU at the same time (different streams with
+ * no ordering between them) overwrite each other's sums and return wrong statistics.  Order such calls
+ * on one stream or with events.
+ *
+ * Errors: DEDISP_EINVAL, DEDISP_ESHAPE (as dedisp_plan_detect), DEDISP_ELIMIT, DEDISP_ECUDA (no device,
+ * more than 64 devices, the address look-up or a launch failed).
+ */
+#define DEDISP_DETECT_STATIC_MAX_SLOTS 18944
+DEDISP_API dedisp_status dedisp_detect_static(const void *out, dedisp_dtype dtype, int ndm, int64_t nsamp_out,
+                                              int64_t out_stride, int nbeams, double nsigma, dedisp_event *events,
+                                              int64_t capacity, dedisp_detect_result *results, void *cuda_stream);
+DEDISP_API int64_t dedisp_detect_static_max_slots(void);
+
  */
 DEDISP_API dedisp_status dedisp_execute_detect(dedisp_plan *plan, const void *in, void *out, dedisp_dtype dtype,
                                                int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,

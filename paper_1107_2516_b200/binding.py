@@ -11,7 +11,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libdedisp_b200.so")
 
-OK, EINVAL, ENOMEM, ECUDA, ESHAPE, ESTATE = range(6)
+OK, EINVAL, ENOMEM, ECUDA, ESHAPE, ESTATE, ELIMIT = range(7)
 F32, U8 = 0, 1
 KERNEL_AUTO, KERNEL_NAIVE, KERNEL_DIRECT, KERNEL_WINDOW, KERNEL_LONG = range(5)
 
@@ -47,6 +47,8 @@ _SIGS = {
     "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
     "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_execute_detect": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
+    "dedisp_detect_static": (_int, [_vp, _int, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
+    "dedisp_detect_static_max_slots": (_i64, []),
     "dedisp_execute_detect_host": (_int, [_vp, _vp, _int, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
     "dedisp_bin": (_int, [_vp, _vp, _i64, _i64, _i64, _i64, _int, _vp]),
@@ -335,6 +337,41 @@ def power_corner_turn(volt, out=None, stream=None):
     import torch
     if not volt.is_cuda or volt.dtype != torch.complex64 or volt.dim() != 2 or volt.stride(1) != 1:
         raise DedispError(ESHAPE, "dedisp_power_corner_turn")
+def detect_static(out, nsigma, capacity=1 << 20, events=None, results=None, stream=None):
+    """dedisp_detect_static: Plan.detect's numbers without a plan and without any allocation inside the
+    library -- for a real-time loop that cannot take cudaMalloc's device-wide stall, or a process whose
+    GPU memory is already fully claimed.  The per-block sums live in a fixed 296 KiB array inside the
+    library (shared by all calls on a GPU: do not overlap two of them), so the shape is limited to
+    nbeams * min(ndm, 1184) <= detect_static_max_slots(); beyond that DedispError(ELIMIT).
+
+    out is a CUDA tensor [(nbeams,) ndm, n] as returned by execute.  Pass preallocated `events`
+    (int32 [nbeams, capacity, 4]) and `results` (float64 [nbeams, 4]) CUDA tensors to keep this wrapper
+    from allocating as well; by default torch allocates them.  Returns (results, events) as Plan.detect."""
+    import torch
+    o = out if out.dim() == 3 else out[None]
+    assert o.is_cuda and o.stride(2) == 1 and o.stride(0) == o.stride(1) * o.shape[1]
+    dt = F32 if o.dtype == torch.float32 else U8
+    nb, ndm = int(o.shape[0]), int(o.shape[1])
+    ev = events if events is not None else torch.zeros((nb, capacity, 4), dtype=torch.int32, device=o.device)
+    res = results if results is not None else torch.zeros((nb, 4), dtype=torch.float64, device=o.device)
+    assert ev.is_contiguous() and ev.dtype == torch.int32 and tuple(ev.shape) == (nb, capacity, 4)
+    assert res.is_contiguous() and res.dtype == torch.float64 and tuple(res.shape) == (nb, 4)
+    _check(lib().dedisp_detect_static(o.data_ptr(), dt, ndm, int(o.shape[2]), int(o.stride(1)), nb, float(nsigma),
+                                      ev.data_ptr(), int(capacity), res.data_ptr(), _stream_ptr(stream)),
+           "dedisp_detect_static")
+    rh = res.cpu().numpy()
+    counts = rh[:, 3].copy().view(np.int64)
+    out_res = [dict(mean=float(rh[b, 0]), sigma=float(rh[b, 1]), threshold=float(rh[b, 2]), count=int(counts[b]))
+               for b in range(nb)]
+    out_ev = [ev[b, :min(int(counts[b]), capacity)].cpu().numpy().view(Plan._REC).reshape(-1) for b in range(nb)]
+    return out_res, out_ev
+
+
+def detect_static_max_slots():
+    """dedisp_detect_static_max_slots: (beam, block) slots of the fixed scratch array."""
+    return int(lib().dedisp_detect_static_max_slots())
+
+
     nsamp, nchans = volt.shape
     if out is None:
         stride = (nsamp + 15) // 16 * 16

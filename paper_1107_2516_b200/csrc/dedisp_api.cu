@@ -1480,3 +1480,4 @@ const char* dedisp_strerror(dedisp_status s)
 const char* dedisp_version(void) { return "dedisp-b200 0.1 (sm_100a)"; }
 
 }  // extern "C"
+    case DEDISP_ELIMIT: return "size exceeds the fixed scratch array of an allocation-free entry point";

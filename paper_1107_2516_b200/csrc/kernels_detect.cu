@@ -6,6 +6,8 @@
 // on scheduling; only the ORDER of the triplets does (an atomic cursor, advanced once per warp and test).
 #include <cuda_runtime.h>
 
+#include <mutex>
+
 #include "dedisp_internal.h"
 
 namespace dedisp {
@@ -272,3 +274,72 @@ int launch_detect(const void* out, Elem t, int nbeams, int ndm, int64_t n, int64
 }
 
 }  // namespace dedisp
+
+// ---- dedisp_detect_static: the two-pass detection above with its per-block partial sums in a fixed
+// array that is part of the library image, for callers that must not allocate (include/dedisp.h).
+namespace dedisp {
+namespace {
+
+// The only scratch the detection needs: two doubles per (beam, block) of detect_stats_kernel.  One copy
+// of this array exists on every GPU that loads the library, from module load until the process exits.
+constexpr int64_t kStaticSlots = DEDISP_DETECT_STATIC_MAX_SLOTS;
+static __device__ __align__(256) double detect_static_scratch[kStaticSlots * 2];
+
+// In host code `detect_static_scratch` is only a handle for the runtime's symbol table, not something a
+// kernel can dereference.  The device address differs per GPU, so it is looked up once per device, with
+// that device current, and remembered here.
+constexpr int kStaticMaxDevices = 64;
+std::mutex static_mu;
+double* static_ptr[kStaticMaxDevices] = {};
+
+cudaError_t static_scratch(double** ptr)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess)
+        return e;
+    if (dev < 0 || dev >= kStaticMaxDevices)
+        return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(static_mu);
+    if (!static_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, detect_static_scratch);
+        if (e != cudaSuccess)
+            return e;
+        if (!p)
+            return cudaErrorInvalidSymbol;
+        static_ptr[dev] = static_cast<double*>(p);
+    }
+    *ptr = static_ptr[dev];
+    return cudaSuccess;
+}
+
+}  // namespace
+}  // namespace dedisp
+
+extern "C" int64_t dedisp_detect_static_max_slots(void) { return dedisp::kStaticSlots; }
+
+extern "C" dedisp_status dedisp_detect_static(const void* out, dedisp_dtype dtype, int ndm, int64_t nsamp_out,
+                                              int64_t out_stride, int nbeams, double nsigma, dedisp_event* events,
+                                              int64_t capacity, dedisp_detect_result* results, void* cuda_stream)
+{
+    using namespace dedisp;
+    if (!out || !results || ndm <= 0 || nbeams <= 0 || nsamp_out <= 0 || capacity < 0 || (capacity > 0 && !events) ||
+        !(nsigma == nsigma) || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
+        return DEDISP_EINVAL;
+    if (out_stride < nsamp_out || out_stride % 4 != 0 || (reinterpret_cast<uintptr_t>(out) & 15) != 0)
+        return DEDISP_ESHAPE;
+    // the fixed array cannot grow: refuse, before touching the device, what does not fit
+    if (static_cast<int64_t>(nbeams) * detect_blocks(ndm) > kStaticSlots)
+        return DEDISP_ELIMIT;
+    double* partial = nullptr;
+    if (static_scratch(&partial) != cudaSuccess)
+        return DEDISP_ECUDA;
+    // Nothing in the array has to start at zero: detect_stats_kernel stores both sums of every slot that
+    // detect_finish_kernel reads, later on the same stream, so whatever an earlier call left is overwritten
+    // first.  The event cursor lives in the caller's `results` and is reset by detect_finish_kernel.
+    int launches = 0;
+    const int rc = launch_detect(out, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, nbeams, ndm, nsamp_out, out_stride,
+                                 nsigma, events, capacity, results, partial, cuda_stream, &launches);
+    return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
+}
