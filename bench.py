@@ -334,7 +334,9 @@ def measure(ctx, cf, args, steps, warmup, primary):
             pass
     plan.set_timing(False)
     kernel_ms = float(np.mean(kms))
-    resolved = plan.resolved_kernel(dtc)
+    # the kernel the timed executes really ran (AUTO is size-aware at execute time: cfg 1 goes to the
+    # one-thread-per-output kernel although the plan's table fits the register-window kernel)
+    resolved = plan.last_kernel
     kname = {dd.KERNEL_WINDOW: "dedisp::window_kernel (all band launches of one execute)",
              dd.KERNEL_DIRECT: "dedisp::direct_kernel", dd.KERNEL_NAIVE: "dedisp::naive_kernel",
              dd.KERNEL_LONG: "dedisp::long_kernel"}.get(resolved, "?")
@@ -549,6 +551,16 @@ def main():
                 "all_configs": others or None,
                 "paper_context": "paper: 50-200x over one Xeon 2.7 GHz core on a Tesla C1060 (PAPER.md:203), ~1.5e10 adds/s",
                 "input_gen_s": res["input_gen_s"]}
+        # compact per-config digest as the LAST key: a record that keeps only the tail of this line still
+        # carries every config's step time, roofline fraction, end-to-end time and the kernel that ran
+        def digest(r):
+            return {"ms": round(r["ms_per_step"], 3), "frac": round(r["roofline"]["frac"], 4),
+                    "kernel": r["resolved_kernel"], "traffic": r["roofline"]["traffic"],
+                    "e2e_ms": round(r["e2e"]["ms_per_step"], 2) if r.get("e2e") else None,
+                    "e2e_events_ms": round(r["e2e_events"]["ms_per_step"], 2) if r.get("e2e_events") else None,
+                    "stage_ms": [round(r["subband"]["stage1_ms"], 3), round(r["subband"]["stage2_ms"], 3)] if r.get("subband") else None}
+        line["summary"] = {args.workload: digest(res)}
+        line["summary"].update({k: digest(v) for k, v in others.items()})
         print(json.dumps(line))
     if world > 1:
         dist.barrier()

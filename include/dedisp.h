@@ -135,7 +135,9 @@ DEDISP_API dedisp_status dedisp_plan_get_subband_shifts(const dedisp_plan *plan,
                                              double *nominal_dm, int32_t *maxshift2);
 
 /* Selects the brute-force kernel (default DEDISP_KERNEL_AUTO).  DEDISP_EINVAL for an unknown
- * value, DEDISP_ESTATE if WINDOW is forced on a plan whose table exceeds its limits. */
+ * value, DEDISP_ESTATE if WINDOW is forced on a plan whose table exceeds its limits.  Scratch is
+ * sized for the kernel selected at the time of dedisp_plan_reserve: after changing the kernel call
+ * dedisp_plan_reserve again (an execute that lacks its scratch returns DEDISP_ESTATE). */
 DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel kernel);
 
 /* Which kernel AUTO resolves to for this plan and dtype (a dedisp_kernel value), -1 on error.  This is
@@ -143,6 +145,12 @@ DEDISP_API dedisp_status dedisp_plan_set_kernel(dedisp_plan *plan, dedisp_kernel
  * register-window tiles than the device has SMs runs the naive kernel (below 8192 outputs per SM) or the
  * direct kernel instead. */
 DEDISP_API int dedisp_plan_resolved_kernel(const dedisp_plan *plan, dedisp_dtype dtype);
+
+/* The kernel the last execute / push on this plan actually ran (a dedisp_kernel value other than AUTO;
+ * subband plans: the kernel of stage 1), -1 before the first execute or if plan is NULL.  Unlike
+ * dedisp_plan_resolved_kernel this reflects AUTO's size rule.  The *_host entries apply that rule once,
+ * to the length of the whole buffer, so all time pieces of one buffer run the same kernel. */
+DEDISP_API int dedisp_plan_last_kernel(const dedisp_plan *plan);
 
 /* Geometry the register-window kernel would use for this plan, 14 int64 to HOST memory:
  * [0] 1 if the plan's table fits the kernel (else the rest is 0), [1] Hb: output samples per
@@ -287,14 +295,6 @@ DEDISP_API dedisp_status dedisp_plan_detect(dedisp_plan *plan, const void *out, 
                                             dedisp_detect_result *results, void *cuda_stream);
 
 /*
- * De-dispersion and event detection in one call (PAPER.md:76 is the step right after the hot path).
- * Arguments as dedisp_execute followed by those of dedisp_plan_detect; `out` still receives the whole
- * de-dispersed buffer.  For brute-force plans that run on the register-window kernel with a single
- * channel band, the kernel's flush accumulates the statistics (fp64 sums of x - pivot and (x - pivot)^2,
- * pivot = sum_c in[c][0], reduced in a fixed order), so detection costs ONE pass over the buffer (the
- * threshold scan) instead of two; other plans run dedisp_execute followed by dedisp_plan_detect.  Same
- * definition of mean / sigma / threshold / events either way.  Asynchronous; needs dedisp_plan_reserve.
-/*
  * dedisp_detect_static -- the event detection of dedisp_plan_detect (same kernels, same
  * definition of mean / sigma / threshold / events, same summation order, hence the same numbers) for
  * callers that cannot let the library allocate device memory.
@@ -344,6 +344,14 @@ DEDISP_API dedisp_status dedisp_detect_static(const void *out, dedisp_dtype dtyp
                                               int64_t capacity, dedisp_detect_result *results, void *cuda_stream);
 DEDISP_API int64_t dedisp_detect_static_max_slots(void);
 
+/*
+ * De-dispersion and event detection in one call (PAPER.md:76 is the step right after the hot path).
+ * Arguments as dedisp_execute followed by those of dedisp_plan_detect; `out` still receives the whole
+ * de-dispersed buffer.  For brute-force plans that run on the register-window kernel with a single
+ * channel band, the kernel's flush accumulates the statistics (fp64 sums of x - pivot and (x - pivot)^2,
+ * pivot = sum_c in[c][0], reduced in a fixed order), so detection costs ONE pass over the buffer (the
+ * threshold scan) instead of two; other plans run dedisp_execute followed by dedisp_plan_detect.  Same
+ * definition of mean / sigma / threshold / events either way.  Asynchronous; needs dedisp_plan_reserve.
  */
 DEDISP_API dedisp_status dedisp_execute_detect(dedisp_plan *plan, const void *in, void *out, dedisp_dtype dtype,
                                                int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
@@ -360,6 +368,15 @@ DEDISP_API dedisp_status dedisp_execute_detect_host(dedisp_plan *plan, const voi
                                                     int64_t nsamp_out, int nbeams, double nsigma,
                                                     dedisp_event *host_events, int64_t capacity,
                                                     dedisp_detect_result *host_results, void *cuda_stream);
+
+/*
+ * Copies the de-dispersed buffer that the last dedisp_execute_host / dedisp_execute_detect_host call on
+ * this plan left on the device (plan-owned; the events-only entry never sends it to the host, so this is
+ * the way to look at the data behind its events) to dst: DEVICE, dense [nbeams][ndm][nsamp_out] float
+ * (DEDISP_F32) or int32 (DEDISP_U8) of that call; `bytes` must be exactly its size (DEDISP_ESHAPE
+ * otherwise).  Asynchronous on cuda_stream.  DEDISP_ESTATE if no host entry has run on the plan.
+ */
+DEDISP_API dedisp_status dedisp_plan_copy_host_output(dedisp_plan *plan, void *dst, int64_t bytes, void *cuda_stream);
 
 /*
  * Power + corner turn, the two steps before de-dispersion in the paper's real-time pipeline

@@ -29,6 +29,7 @@ _SIGS = {
     "dedisp_plan_get_subband_shifts": (_int, [_vp, _vp, _vp, _vp, _vp]),
     "dedisp_plan_set_kernel": (_int, [_vp, _int]),
     "dedisp_plan_resolved_kernel": (_int, [_vp, _int]),
+    "dedisp_plan_last_kernel": (_int, [_vp]),
     "dedisp_plan_window_info": (_int, [_vp, _vp]),
     "dedisp_plan_set_window_geometry": (_int, [_vp, _int, _int, _int, _int]),
     "dedisp_plan_reserve": (_int, [_vp, _int, _i64, _int]),
@@ -46,9 +47,10 @@ _SIGS = {
     "dedisp_plan_last_kernel_ms": (_int, [_vp, _vp]),
     "dedisp_plan_last_stage_ms": (_int, [_vp, _vp]),
     "dedisp_plan_detect": (_int, [_vp, _vp, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
-    "dedisp_execute_detect": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_detect_static": (_int, [_vp, _int, _int, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_detect_static_max_slots": (_i64, []),
+    "dedisp_execute_detect": (_int, [_vp, _vp, _vp, _int, _i64, _i64, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
+    "dedisp_plan_copy_host_output": (_int, [_vp, _vp, _i64, _vp]),
     "dedisp_execute_detect_host": (_int, [_vp, _vp, _int, _i64, _int, _dbl, _vp, _i64, _vp, _vp]),
     "dedisp_power_corner_turn": (_int, [_vp, _vp, _int, _i64, _i64, _i64, _vp]),
     "dedisp_bin": (_int, [_vp, _vp, _i64, _i64, _i64, _i64, _int, _vp]),
@@ -128,15 +130,15 @@ class Plan:
     def reserve(self, dtype, nsamp_out, nbeams=1):
         """dedisp_plan_reserve: tables onto the current device, scratch for this shape (blocking)."""
         _check(lib().dedisp_plan_reserve(self._h, int(dtype), int(nsamp_out), int(nbeams)), "dedisp_plan_reserve")
-        n, b = self._reserved.get(int(dtype), (0, 0))
-        self._reserved[int(dtype)] = (max(n, int(nsamp_out)), max(b, int(nbeams)))
+        # the library's buffers only grow and their sizes rise with both arguments, so a shape is covered
+        # exactly when ONE earlier reserve had both at least as large (not the maxima taken separately)
+        self._reserved.setdefault(int(dtype), []).append((int(nsamp_out), int(nbeams)))
 
     def _ensure_reserved(self, dtype, nsamp_out, nbeams):
         # execute / detect never allocate (include/dedisp.h): the binding reserves the first time a
         # shape is seen, which keeps `plan.execute(x, n)` a one-liner
-        n, b = self._reserved.get(int(dtype), (-1, 0))
-        if nsamp_out > n or nbeams > b:
-            self.reserve(dtype, max(n, int(nsamp_out)), max(b, int(nbeams)))
+        if not any(n >= nsamp_out and b >= nbeams for n, b in self._reserved.get(int(dtype), ())):
+            self.reserve(dtype, int(nsamp_out), int(nbeams))
 
     def close(self):
         if getattr(self, "_h", None):
@@ -212,6 +214,11 @@ class Plan:
     @property
     def last_launches(self):
         return int(lib().dedisp_plan_last_launches(self._h))
+
+    @property
+    def last_kernel(self):
+        """dedisp_plan_last_kernel: the kernel the last execute / push really ran (KERNEL_*), -1 before any."""
+        return int(lib().dedisp_plan_last_kernel(self._h))
 
     def execute(self, x, nsamp_out, out=None, stream=None):
         """x: CUDA tensor [nchans][n_in] or [nbeams][nchans][n_in] (float32 or uint8), last dim
@@ -316,6 +323,16 @@ class Plan:
         ev = ea.view(np.uint8).reshape(nb, -1)[:, :capacity * 16].view(self._REC).reshape(nb, capacity)
         return results, [ev[b, :min(int(counts[b]), capacity)] for b in range(nb)]
 
+    def host_output(self, nbeams, nsamp_out, dtype=F32, stream=None):
+        """dedisp_plan_copy_host_output: the de-dispersed buffer of the last execute_host /
+        execute_detect_host call as a CUDA tensor [nbeams][ndm][nsamp_out] (a copy)."""
+        import torch
+        t = torch.empty((int(nbeams), self.ndm, int(nsamp_out)), dtype=torch.float32 if dtype == F32 else torch.int32,
+                        device="cuda")
+        _check(lib().dedisp_plan_copy_host_output(self._h, t.data_ptr(), t.numel() * 4, _stream_ptr(stream)),
+               "dedisp_plan_copy_host_output")
+        return t
+
     def execute_host(self, x, nsamp_out, out=None, stream=None):
         """x: numpy / CPU tensor [nbeams][nchans][nsamp_out+max_delay] dense; returns numpy out."""
         xa = x.numpy() if hasattr(x, "numpy") else np.asarray(x)
@@ -331,12 +348,6 @@ class Plan:
         return out
 
 
-def power_corner_turn(volt, out=None, stream=None):
-    """dedisp_power_corner_turn: volt CUDA complex64 [nsamp][nchans] (row stride free) -> float32
-    [nchans][nsamp] in the de-disperser's layout (row stride padded to 16 elements)."""
-    import torch
-    if not volt.is_cuda or volt.dtype != torch.complex64 or volt.dim() != 2 or volt.stride(1) != 1:
-        raise DedispError(ESHAPE, "dedisp_power_corner_turn")
 def detect_static(out, nsigma, capacity=1 << 20, events=None, results=None, stream=None):
     """dedisp_detect_static: Plan.detect's numbers without a plan and without any allocation inside the
     library -- for a real-time loop that cannot take cudaMalloc's device-wide stall, or a process whose
@@ -372,6 +383,12 @@ def detect_static_max_slots():
     return int(lib().dedisp_detect_static_max_slots())
 
 
+def power_corner_turn(volt, out=None, stream=None):
+    """dedisp_power_corner_turn: volt CUDA complex64 [nsamp][nchans] (row stride free) -> float32
+    [nchans][nsamp] in the de-disperser's layout (row stride padded to 16 elements)."""
+    import torch
+    if not volt.is_cuda or volt.dtype != torch.complex64 or volt.dim() != 2 or volt.stride(1) != 1:
+        raise DedispError(ESHAPE, "dedisp_power_corner_turn")
     nsamp, nchans = volt.shape
     if out is None:
         stride = (nsamp + 15) // 16 * 16

@@ -88,8 +88,11 @@ struct dedisp_plan {
     DevBuf det_partial;        // dedisp_plan_detect / dedisp_execute_detect workspace (per-block partial sums)
     DevBuf det_pivot;          // [nbeams] doubles
     DevBuf det_events, det_results;  // device staging of dedisp_execute_detect_host
+    // shape of the de-dispersed data the last *_host entry left in host_out: rows of ho_n samples, ho_stride apart
+    int64_t ho_rows = 0, ho_n = 0, ho_stride = 0;
     dedisp_kernel kernel = DEDISP_KERNEL_AUTO;
     int last_launches = 0;
+    int last_kernel = -1;  // dedisp_kernel the last execute ran (subband plans: stage 1's), -1 before the first
     int nstreams = 0;
     // register-window kernel (brute-force plans): host plan, device tables, pair scratch
     WindowPlan win;
@@ -303,22 +306,30 @@ dedisp_status run_window(dedisp_plan* plan, const void* in, void* out, Elem in_t
         g = g < 1 ? 1 : g > plan->win.ntile_dm ? plan->win.ntile_dm : g;
         a.dm_group = g > plan->win.ntile_dm ? plan->win.ntile_dm : g;
     }
+    plan->last_kernel = DEDISP_KERNEL_WINDOW;
     return launch_window(a, in_t, stream, &plan->last_launches) == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
 int run_problem(dedisp_plan* plan, const Problem& pr, Elem in_t, const int spread[3], void* stream)
 {
     switch (plan->kernel) {
-    case DEDISP_KERNEL_NAIVE: return launch_naive(pr, in_t, stream, &plan->last_launches);
-    case DEDISP_KERNEL_DIRECT: return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
+    case DEDISP_KERNEL_NAIVE:
+        plan->last_kernel = DEDISP_KERNEL_NAIVE;
+        return launch_naive(pr, in_t, stream, &plan->last_launches);
+    case DEDISP_KERNEL_DIRECT:
+        plan->last_kernel = DEDISP_KERNEL_DIRECT;
+        return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
     default: {
         // long tiles pay once a row has a few tiles' worth of samples; short problems keep the
         // 256-sample tiles of the direct kernel
         if (plan->kernel == DEDISP_KERNEL_LONG || pr.n_out >= 4096) {
             const int rc = launch_long(pr, in_t, spread[1], stream, &plan->last_launches);
-            if (rc != -1)
+            if (rc != -1) {
+                plan->last_kernel = DEDISP_KERNEL_LONG;
                 return rc;
+            }
         }
+        plan->last_kernel = DEDISP_KERNEL_DIRECT;
         return launch_direct(pr, in_t, spread, stream, &plan->last_launches);
     }
     }
@@ -326,8 +337,11 @@ int run_problem(dedisp_plan* plan, const Problem& pr, Elem in_t, const int sprea
 
 dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedisp_dtype dtype,
                              int64_t nsamp_out, int64_t in_stride, int64_t out_stride, int nbeams,
-                             void* stream, const StatReq* sr = nullptr)
+                             void* stream, const StatReq* sr = nullptr, int64_t policy_len = 0)
 {
+    // policy_len > 0: the host entries cut one buffer into time pieces and pass the length of the WHOLE
+    // buffer here, so that AUTO's size rule picks one kernel for all pieces (one fp32 summation order per
+    // output buffer) instead of judging every piece by its own length
     if (!plan || nbeams <= 0 || nsamp_out < 0 || (dtype != DEDISP_F32 && dtype != DEDISP_U8))
         return DEDISP_EINVAL;
     if (nsamp_out == 0) {
@@ -362,8 +376,9 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     // ~8192 outputs per SM, the direct kernel's 8..32 rows x 256 samples beyond (measured on cfg 1:
     // naive 0.037 ms, direct 0.054 ms, window 0.069 ms, long 0.078 ms).
     bool small = false;
+    const int64_t size_len = policy_len > 0 ? policy_len : nsamp_out;
     if (plan->kernel == DEDISP_KERNEL_AUTO && plan->nsub == 0 && !sr && use_window(plan, dtype, nsamp_out))
-        small = static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nsamp_out) * nbeams < plan->nsm;
+        small = static_cast<int64_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, size_len) * nbeams < plan->nsm;
     if (!small && use_window(plan, dtype, nsamp_out))
         return run_window(plan, in, out, in_t, nsamp_out, in_stride, out_stride, nbeams, stream, sr);
     if (sr)
@@ -398,7 +413,8 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
         pr.ndm = plan->ndm;
         pr.nb1 = 1;
         if (small) {
-            const bool tiny = static_cast<int64_t>(plan->ndm) * nsamp_out * nbeams < 8192LL * plan->nsm;
+            const bool tiny = static_cast<int64_t>(plan->ndm) * size_len * nbeams < 8192LL * plan->nsm;
+            plan->last_kernel = tiny ? DEDISP_KERNEL_NAIVE : DEDISP_KERNEL_DIRECT;
             rc = tiny ? launch_naive(pr, in_t, stream, &plan->last_launches)
                       : launch_direct(pr, in_t, plan->spread_full, stream, &plan->last_launches);
         } else {
@@ -460,7 +476,9 @@ dedisp_status execute_device(dedisp_plan* plan, const void* in, void* out, dedis
     p2.ndm = plan->nfine;
     p2.nb0 = nbeams;
     p2.nb1 = ncoarse;
+    const int stage1_kernel = plan->last_kernel;
     rc = run_problem(plan, p2, dtype == DEDISP_F32 ? Elem::F32 : Elem::I32, plan->spread_s2, stream);
+    plan->last_kernel = stage1_kernel;
     return rc == 0 ? DEDISP_OK : DEDISP_ECUDA;
 }
 
@@ -473,15 +491,31 @@ dedisp_status reserve(dedisp_plan* plan, dedisp_dtype dtype, int64_t nsamp_out, 
     if (st != DEDISP_OK)
         return st;
     size_t pairs = 0, scratch = 0;
+    int64_t nwin = 0;  // longest execute <= nsamp_out that runs on the register-window kernel
     if (plan->nsub == 0) {
-        if (use_window(plan, dtype, nsamp_out) && nsamp_out > 0)
-            pairs = static_cast<size_t>(nbeams) * plan->nchans * window_pair_stride(plan->win, nsamp_out) * 8;
+        // The reservation covers every execute of UP TO nsamp_out samples.  A length beyond the window
+        // kernel's 32-bit time limit runs on the long-tile kernel, but shorter executes of the same plan
+        // still resolve to the window kernel: size the pair buffer for the longest length it accepts
+        // (window_pair_stride grows with the length, so that one covers all shorter ones).
+        if (nsamp_out > 0 && use_window(plan, dtype, 0)) {
+            nwin = nsamp_out;
+            if (!use_window(plan, dtype, nwin)) {
+                int64_t lo = 0, hi = nsamp_out;  // accepted at lo, refused at hi
+                while (hi - lo > 1) {
+                    const int64_t mid = lo + (hi - lo) / 2;
+                    (use_window(plan, dtype, mid) ? lo : hi) = mid;
+                }
+                nwin = lo;
+            }
+        }
+        if (nwin > 0)
+            pairs = static_cast<size_t>(nbeams) * plan->nchans * window_pair_stride(plan->win, nwin) * 8;
     } else {
         scratch = static_cast<size_t>(dedisp_plan_scratch_bytes(plan, nsamp_out, nbeams));
     }
     size_t npart = static_cast<size_t>(detect_blocks(plan->ndm));
-    if (fused_stats_ok(plan, dtype, nsamp_out) && nsamp_out > 0)
-        npart = std::max(npart, static_cast<size_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nsamp_out));
+    if (nwin > 0 && fused_stats_ok(plan, dtype, nwin))
+        npart = std::max(npart, static_cast<size_t>(plan->win.ntile_dm) * window_ntile_t(plan->win, nwin));
     const size_t det = static_cast<size_t>(nbeams) * npart * 2 * sizeof(double);
     if (plan->pairs.ensure(pairs) != cudaSuccess || plan->scratch.ensure(scratch) != cudaSuccess ||
         plan->det_partial.ensure(det) != cudaSuccess || plan->det_pivot.ensure(nbeams * sizeof(double)) != cudaSuccess) {
@@ -489,6 +523,17 @@ dedisp_status reserve(dedisp_plan* plan, dedisp_dtype dtype, int64_t nsamp_out, 
         return DEDISP_ENOMEM;
     }
     return DEDISP_OK;
+}
+
+// Error exit of the host entries: waits for the two copy streams and the caller's stream (errors ignored,
+// the call is failing already) so that no DMA touches the caller's host buffers after the return.
+void drain_host_streams(dedisp_plan* plan, cudaStream_t st)
+{
+    for (cudaStream_t q : {plan->copy_st[0], plan->copy_st[1]})
+        if (q)
+            cudaStreamSynchronize(q);
+    cudaStreamSynchronize(st);
+    cudaGetLastError();
 }
 
 // Time piece i of a host-entry execute: uniform pieces of csize samples, the first one split at a quarter so
@@ -640,7 +685,23 @@ int dedisp_plan_nchans(const dedisp_plan* p) { return p ? p->nchans : -1; }
 int dedisp_plan_ndm(const dedisp_plan* p) { return p ? p->ndm : -1; }
 int dedisp_plan_nsub(const dedisp_plan* p) { return p ? p->nsub : -1; }
 int dedisp_plan_nfine(const dedisp_plan* p) { return p ? p->nfine : -1; }
+int dedisp_plan_last_kernel(const dedisp_plan* p) { return p ? p->last_kernel : -1; }
+
 int dedisp_plan_last_launches(const dedisp_plan* p) { return p ? p->last_launches : -1; }
+
+dedisp_status dedisp_plan_copy_host_output(dedisp_plan* p, void* dst, int64_t bytes, void* cuda_stream)
+{
+    if (!p || !dst)
+        return DEDISP_EINVAL;
+    if (p->ho_rows == 0 || !p->host_out.p)
+        return DEDISP_ESTATE;
+    if (bytes != p->ho_rows * p->ho_n * 4)
+        return DEDISP_ESHAPE;
+    return cudaMemcpy2DAsync(dst, p->ho_n * 4, p->host_out.p, p->ho_stride * 4, p->ho_n * 4, p->ho_rows,
+                             cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)) == cudaSuccess
+               ? DEDISP_OK
+               : DEDISP_ECUDA;
+}
 
 dedisp_status dedisp_plan_set_timing(dedisp_plan* p, int on)
 {
@@ -815,6 +876,9 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
         cudaGetLastError();
         return DEDISP_ENOMEM;
     }
+    plan->ho_rows = static_cast<int64_t>(rows_out);
+    plan->ho_n = nsamp_out;
+    plan->ho_stride = out_stride;
     // Brute-force plans are cut into up to kHostChunks time chunks so that the H2D copy of chunk
     // i+1, the kernels of chunk i and the D2H copy of chunk i-1 overlap (outputs of different times
     // are independent; chunk i reads input columns [t_i, t_i + C_i + max_delay)).
@@ -833,14 +897,15 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
         if (cudaMemcpy2DAsync(plan->host_in.p, in_stride * es, host_in, n_in * es, n_in * es, rows_in,
                               cudaMemcpyHostToDevice, st) != cudaSuccess)
             return DEDISP_ECUDA;
+        // from here on a copy that reads the caller's host_in may be queued: no return without waiting for it
         dedisp_status s = execute_device(plan, plan->host_in.p, plan->host_out.p, dtype, nsamp_out,
                                          in_stride, out_stride, nbeams, cuda_stream);
-        if (s != DEDISP_OK)
-            return s;
-        if (cudaMemcpy2DAsync(host_out, nsamp_out * 4, plan->host_out.p, out_stride * 4, nsamp_out * 4,
-                              rows_out, cudaMemcpyDeviceToHost, st) != cudaSuccess)
-            return DEDISP_ECUDA;
-        return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
+        if (s == DEDISP_OK && cudaMemcpy2DAsync(host_out, nsamp_out * 4, plan->host_out.p, out_stride * 4, nsamp_out * 4,
+                                                rows_out, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            s = DEDISP_ECUDA;
+        if (cudaStreamSynchronize(st) != cudaSuccess && s == DEDISP_OK)
+            s = DEDISP_ECUDA;
+        return s;
     }
     if (!ensure_copy_streams(plan))
         return DEDISP_ECUDA;
@@ -859,6 +924,7 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
     char* hout = static_cast<char*>(host_out);
     int launches = 0;
     int64_t col = 0;  // input columns copied so far
+    dedisp_status exec_status = DEDISP_OK;
     for (int i = 0; i <= nchunk && ok; ++i) {
         int64_t t0, cn;
         if (!host_piece(nsamp_out, csize, i, &t0, &cn))
@@ -872,20 +938,23 @@ dedisp_status dedisp_execute_host(dedisp_plan* plan, const void* host_in, void* 
         ok = ok && cudaEventRecord(ev_in[i], h2d) == cudaSuccess && cudaStreamWaitEvent(st, ev_in[i], 0) == cudaSuccess;
         if (!ok)
             break;
-        const dedisp_status s = execute_device(plan, din + t0 * es, dout + t0 * 4, dtype, cn, in_stride,
-                                               out_stride, nbeams, cuda_stream);
-        if (s != DEDISP_OK)
-            return s;
+        exec_status = execute_device(plan, din + t0 * es, dout + t0 * 4, dtype, cn, in_stride,
+                                     out_stride, nbeams, cuda_stream, nullptr, nsamp_out);
+        if (exec_status != DEDISP_OK)
+            break;
         launches += plan->last_launches;
         ok = cudaEventRecord(ev_ex[i], st) == cudaSuccess && cudaStreamWaitEvent(d2h, ev_ex[i], 0) == cudaSuccess &&
              cudaMemcpy2DAsync(hout + t0 * 4, nsamp_out * 4, dout + t0 * 4, out_stride * 4, cn * 4, rows_out,
                                cudaMemcpyDeviceToHost, d2h) == cudaSuccess;
     }
     plan->last_launches = launches;
+    ok = ok && exec_status == DEDISP_OK;
     ok = ok && cudaEventRecord(ev_done, d2h) == cudaSuccess && cudaStreamWaitEvent(st, ev_done, 0) == cudaSuccess;
     if (!ok) {
-        cudaGetLastError();
-        return DEDISP_ECUDA;
+        // copies from / to the caller's buffers may still be queued on the private streams, which the
+        // caller's stream has not joined: wait for all three before the buffers go back to the caller
+        drain_host_streams(plan, st);
+        return exec_status != DEDISP_OK ? exec_status : DEDISP_ECUDA;
     }
     return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
 }
@@ -1030,9 +1099,11 @@ dedisp_status dedisp_stream_push_host(dedisp_stream* s, const void* host_chunk_i
         if (!ok)
             break;
         const dedisp_status r = execute_device(p, cur + t0 * es, dout + t0 * 4, s->dtype, cn, s->wstride, C,
-                                               s->nbeams, cuda_stream);
-        if (r != DEDISP_OK)
+                                               s->nbeams, cuda_stream, nullptr, C);
+        if (r != DEDISP_OK) {
+            drain_host_streams(p, st);  // copies of the caller's chunk / into the caller's out may be queued
             return r;
+        }
         launches += p->last_launches;
         ok = cudaEventRecord(ev_ex[j], st) == cudaSuccess && cudaStreamWaitEvent(d2h, ev_ex[j], 0) == cudaSuccess &&
              cudaMemcpy2DAsync(hout + t0 * 4, C * 4, dout + t0 * 4, C * 4, cn * 4, rows_out, cudaMemcpyDeviceToHost,
@@ -1046,7 +1117,7 @@ dedisp_status dedisp_stream_push_host(dedisp_stream* s, const void* host_chunk_i
     s->cur ^= 1;
     ok = ok && cudaEventRecord(ev_done, d2h) == cudaSuccess && cudaStreamWaitEvent(st, ev_done, 0) == cudaSuccess;
     if (!ok) {
-        cudaGetLastError();
+        drain_host_streams(p, st);
         return DEDISP_ECUDA;
     }
     return cudaStreamSynchronize(st) == cudaSuccess ? DEDISP_OK : DEDISP_ECUDA;
@@ -1163,6 +1234,9 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
         cudaGetLastError();
         return DEDISP_ENOMEM;
     }
+    plan->ho_rows = static_cast<int64_t>(rows_out);
+    plan->ho_n = nsamp_out;
+    plan->ho_stride = out_stride;
     // time pieces as in dedisp_execute_host: the H2D copy of piece i+1 overlaps the kernels of piece i; nothing
     // but the events and 32 bytes of statistics per beam comes back
     int nchunk = 1;
@@ -1198,6 +1272,7 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
     const Elem in_t = dtype == DEDISP_F32 ? Elem::F32 : Elem::U8;
     int launches = 0;
     int64_t col = 0, part_off = 0;
+    dedisp_status exec_status = DEDISP_OK;
     for (int i = 0; i <= nchunk && ok; ++i) {
         int64_t t0 = 0, cn = nsamp_out;
         if (nchunk == 1 ? i > 0 : !host_piece(nsamp_out, csize, i, &t0, &cn))
@@ -1211,19 +1286,23 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
         ok = ok && cudaEventRecord(ev_in[i], h2d) == cudaSuccess && cudaStreamWaitEvent(st, ev_in[i], 0) == cudaSuccess;
         if (!ok)
             break;
-        if (i == 0 && fused && launch_detect_pivot(din, in_t, nbeams, plan->nchans, in_stride, pivot, cuda_stream, &launches) != 0)
-            return DEDISP_ECUDA;
+        if (i == 0 && fused && launch_detect_pivot(din, in_t, nbeams, plan->nchans, in_stride, pivot, cuda_stream, &launches) != 0) {
+            ok = false;
+            break;
+        }
         const StatReq sr{pivot, static_cast<double*>(plan->det_partial.p), npart_total, part_off};
-        const dedisp_status s = execute_device(plan, din + t0 * es, dout + t0 * 4, dtype, cn, in_stride, out_stride, nbeams,
-                                               cuda_stream, fused ? &sr : nullptr);
-        if (s != DEDISP_OK)
-            return s;
+        exec_status = execute_device(plan, din + t0 * es, dout + t0 * 4, dtype, cn, in_stride, out_stride, nbeams,
+                                     cuda_stream, fused ? &sr : nullptr, nsamp_out);
+        if (exec_status != DEDISP_OK)
+            break;
         launches += plan->last_launches;
         part_off += static_cast<int64_t>(plan->win.ntile_dm) * (fused ? window_ntile_t(plan->win, cn) : 0);
     }
-    if (!ok) {
-        cudaGetLastError();
-        return DEDISP_ECUDA;
+    if (!ok || exec_status != DEDISP_OK) {
+        // host-to-device copies that read the caller's host_in may still be queued on the private copy
+        // stream: wait for them before the buffer goes back to the caller
+        drain_host_streams(plan, st);
+        return exec_status != DEDISP_OK ? exec_status : DEDISP_ECUDA;
     }
     dedisp_event* dev = static_cast<dedisp_event*>(plan->det_events.p);
     dedisp_detect_result* dres = static_cast<dedisp_detect_result*>(plan->det_results.p);
@@ -1240,14 +1319,14 @@ dedisp_status dedisp_execute_detect_host(dedisp_plan* plan, const void* host_in,
     if (rc != 0 ||
         cudaMemcpyAsync(host_results, dres, nbeams * sizeof(dedisp_detect_result), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
         cudaStreamSynchronize(st) != cudaSuccess) {
-        cudaGetLastError();
+        drain_host_streams(plan, st);
         return DEDISP_ECUDA;
     }
     for (int b = 0; b < nbeams; ++b) {
         const int64_t k = std::min<int64_t>(host_results[b].count, capacity);
         if (k > 0 && cudaMemcpyAsync(host_events + static_cast<int64_t>(b) * capacity, dev + static_cast<int64_t>(b) * capacity,
                                      k * sizeof(dedisp_event), cudaMemcpyDeviceToHost, st) != cudaSuccess) {
-            cudaGetLastError();
+            drain_host_streams(plan, st);
             return DEDISP_ECUDA;
         }
     }
@@ -1473,6 +1552,7 @@ const char* dedisp_strerror(dedisp_status s)
     case DEDISP_ECUDA: return "CUDA error";
     case DEDISP_ESHAPE: return "shape, stride or alignment does not match the plan";
     case DEDISP_ESTATE: return "call not valid for this plan or stream";
+    case DEDISP_ELIMIT: return "size exceeds the fixed scratch array of an allocation-free entry point";
     }
     return "unknown status";
 }
@@ -1480,4 +1560,3 @@ const char* dedisp_strerror(dedisp_status s)
 const char* dedisp_version(void) { return "dedisp-b200 0.1 (sm_100a)"; }
 
 }  // extern "C"
-    case DEDISP_ELIMIT: return "size exceeds the fixed scratch array of an allocation-free entry point";

@@ -103,8 +103,9 @@ struct WindowPlan {
     int Hb = 0;         // output samples per block and row: 2 * NT * W - kmax (blocks are Hb samples apart)
     int kmax = 0;       // largest number of row shifts of a row inside one band
     int lmax = 0;       // longest staged channel segment, in pairs
-    // ring of the staged segments (window_ring): ch channels per pipeline stage, nst stages of
-    // { hdr_words header words, ch slots of slot_bytes }; nst = 0: the segments do not fit shared memory
+    // ring of the staged segments (sized at the end of build_window_plan): ch channels per pipeline stage,
+    // nst >= 2 stages of { hdr_words header words, ch slots of slot_bytes }; nst = 0: the segments do not fit
+    // shared memory.  The kernel stages with P = min(4, nst) producer warps, so a ring of 2 or 3 cannot be lapped.
     int ch = 0, nst = 0, slot_bytes = 0, hdr_words = 0;
     int ntile_dm = 0;
     int nband = 0;

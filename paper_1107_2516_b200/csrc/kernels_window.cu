@@ -241,7 +241,18 @@ __global__ void __launch_bounds__((G * NT + 4) * 32, (G * NT == 4 ? 2 : 1))
     constexpr int kPool = ((NCW == 4 ? 32768 : 65536) - 4 * 32 * 24) / (NCW * 32) / 8 * 8;
     constexpr int kConsRegs = kPool > 240 ? 240 : kPool;
     static_assert(NCW % 4 == 0, "setmaxnreg works on groups of four warps");
-    static_assert(NCW <= 12 && D <= kWinD, "hand-over area; shapes with 16 consumer warps (120 registers each) hung in a trial and are not supported");
+    // setmaxnreg.inc waits until the registers are free in the BLOCK's pool, and that pool is what the block
+    // was launched with: threads x the per-thread count ptxas derives from __launch_bounds__ (the largest
+    // multiple of 8 that lets the stated number of blocks fit 64 K registers -- cuobjdump -res-usage shows
+    // 128 for 512 threads, 168 for 384), not the whole register file.  The consumers' kConsRegs and the
+    // producers' 24 must fit it, or the consumers wait for ever.  This is what hung the 16-consumer-warp
+    // shapes tried in round 2: 640 threads launch with 96 registers = 61 440, and 512 x 120 + 128 x 24 = 64 512.
+    // (They could run with 112, which does not hold D x T >= 60 pairs, so no such shape is instantiated.)
+    constexpr int kThreads = (NCW + 4) * 32, kBlocksPerSm = NCW == 4 ? 2 : 1;
+    constexpr int kLaunchRegs = 65536 / (kThreads * kBlocksPerSm) / 8 * 8 > 255 ? 255 : 65536 / (kThreads * kBlocksPerSm) / 8 * 8;
+    static_assert(NCW * 32 * kConsRegs + 4 * 32 * 24 <= kThreads * kLaunchRegs,
+                  "setmaxnreg.inc would never be granted: consumer + producer registers exceed the block's launch pool");
+    static_assert(NCW <= 12 && D <= kWinD, "hand-over area holds 16 warps, but 16 consumer warps leave 112 registers each (see above)");
     extern __shared__ __align__(128) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // Block order: groups of a.dm_group DM tiles; inside a group all time tiles, DM tile fastest.

@@ -124,6 +124,7 @@ def test_null_handles_and_misc():
     with pytest.raises(dd.DedispError):
         p.set_kernel(17)
     assert p.resolved_kernel() in (dd.KERNEL_DIRECT, dd.KERNEL_WINDOW)
+    assert p.last_kernel == -1 and dd.lib().dedisp_plan_last_kernel(None) == -1     # nothing executed yet
     p.set_kernel(dd.KERNEL_NAIVE)
     assert p.resolved_kernel() == dd.KERNEL_NAIVE
 

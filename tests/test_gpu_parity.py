@@ -171,6 +171,8 @@ def test_window_geometries(oracle, geom):
     info = plan.window_info()
     assert info["ok"] == 1 and (info["T"], info["G"], info["NT"], info["D"]) == geom
     assert info["kmax"] > 0 and info["Hb"] == (2 * NT * 32 * T - info["kmax"]) // 2 * 2
+    # shallow rings, served by min(4, stages) producer warps: 3 stages with these shapes, 2 with the others
+    assert info["ring_stages"] == (3 if geom in ((21, 8, 1, 4), (11, 6, 2, 5), (9, 6, 2, 6)) else 2)
     plan.set_kernel(dd.KERNEL_WINDOW)
     got = plan.execute(to_dev(x), cf.n_out).cpu().numpy()
     assert plan.last_launches == 1 + info["nband"]
@@ -353,6 +355,15 @@ def test_execute_detect_fused(oracle, dtype):
             c = set(map(tuple, ev.tolist()))
             for (t, d) in a ^ c:
                 assert abs(host[b][d, t] - thr) <= 1e-5 * np.abs(x[b]).sum(axis=0).max()
+        # the buffer behind those events (it never left the device): every element against the oracle, and
+        # the returned events are exactly oracle.detect's on THAT buffer
+        hbuf = plan.host_output(2, cf.n_out, dd.F32).cpu().numpy()
+        for b in range(2):
+            ref, sa = oracle.brute_f32(x[b], tab, cf.n_out)
+            check_f32(hbuf[b], ref, sa)
+        _check_detect(oracle, hbuf, rh, eh, nsig, cap)
+    with pytest.raises(dd.DedispError):
+        plan.host_output(3, cf.n_out)                    # not the shape of the last host call
     plan.close()
     # unfused route (subband plan), same definition
     cs = small_cfg(dtype, nchans=128, ndm=96, n_out=2048 + 33, step=0.25, nsub=8, nfine=12)
@@ -605,16 +616,38 @@ def test_cfg4_full_size_seeded(oracle):
     out = plan.execute(xd[:, :n_in], cf.n_out)
     assert plan.last_launches == 2
     got = out.cpu().numpy()
-    del out, xd
+    del out
+    # (4) BRUTE FORCE on the GPU on the same input (BASELINE cfg 4: "also compared against brute force on the
+    # same input"): brute-force plans on rows of 4096 channels whose input buffer has 2.28e9
+    # elements (> 2^31: 64-bit row offsets) and whose max_delay 424 712 exceeds n_out 131 072.  The direct
+    # kernel on the 128 nominal trials + the last 16 (rows 32 DM steps apart: too far for shared staging of the
+    # long-tile kernel, which AUTO would therefore not pick), the long-tile kernel on the last 32 contiguous ones.
+    nominal = np.arange(tab.ncoarse) * cf.nfine + cf.nfine // 2
+    subsets = {"direct": np.concatenate([nominal, np.arange(cf.ndm - 16, cf.ndm)]), "long": np.arange(cf.ndm - 32, cf.ndm)}
+    assert cf.nchans * stride > 2 ** 31 and int(full.max()) > cf.n_out
+    brute = {}
+    for kname, rows in subsets.items():
+        bargs = cf.plan_args()
+        bargs.update(dm_list=np.asarray(cf.dm_list)[rows], nsub=0, nfine=0)
+        bp = dd.Plan(**bargs)
+        assert (bp.shifts() == full[rows]).all() and bp.max_delay == int(full.max())
+        bp.set_kernel(KERNELS[kname])
+        brute[kname] = bp.execute(xd[:, :n_in], cf.n_out).cpu().numpy()
+        assert bp.last_kernel == KERNELS[kname] and bp.last_launches == 1
+        bp.close()
+    del xd
     torch.cuda.empty_cache()
+    for kname, rows in subsets.items():
+        ref, sa = oracle.brute_f32(x, full[rows], cf.n_out)
+        check_f32(brute[kname], ref, sa)
+        if kname == "direct":
+            bref, bsa = ref, sa
     # (1) subband GPU vs subband oracle, every output of four groups
     for k in (0, 1, 64, 127):
         ref, sa = oracle.subband(x, tab, cf.n_out, groups=[k])
         check_f32(got[k * cf.nfine:(k + 1) * cf.nfine], ref, sa)
     # (2) nominal rows equal brute force (reading R8)
-    nominal = np.arange(tab.ncoarse) * cf.nfine + cf.nfine // 2
-    ref, sa = oracle.brute_f32(x, full[nominal], cf.n_out)
-    check_f32(got[nominal], ref, sa)
+    check_f32(got[nominal], bref[:len(nominal)], bsa[:len(nominal)])
     # (3) pulses
     for i, (trial, t0, w, amp) in enumerate(pulses):
         k = trial // cf.nfine
@@ -841,3 +874,98 @@ def test_execute_is_asynchronous_and_allocation_free(oracle):
     assert (out.cpu().numpy() == oracle.brute_u8(x[0], tab, cf.n_out)).all()
     st = L.dedisp_execute(plan._h, xd.data_ptr(), out.data_ptr(), dd.U8, 2 * cf.n_out, xd.stride(0), 2 * cf.n_out, 1, 0)
     assert st in (dd.binding.ESTATE, dd.binding.ESHAPE)              # beyond the reservation / the input
+
+
+def test_reserve_covers_shorter_executes_and_binding_bookkeeping(oracle):
+    """dedisp_plan_reserve promises executes of UP TO nsamp_out samples (include/dedisp.h).  (i) A reserve
+    beyond the register-window kernel's 32-bit time limit (2 channels x 2^30 samples: 17 GB of pair
+    scratch) must still size the pair buffer for the shorter executes that resolve to that kernel.
+    (ii) The binding must not take reserve(100, 4 beams) + reserve(1000, 1 beam) for a reservation of
+    1000 samples x 4 beams."""
+    dm = np.arange(16) * 0.4
+    plan = dd.Plan(2, 150.0, 0.1, 0.2, dm)
+    plan.reserve(dd.F32, (1 << 30) + 4096, 1)
+    assert plan.resolved_kernel(dd.F32) == dd.KERNEL_WINDOW
+    tab = oracle.shift_table(2, 150.0, 0.1, 0.2, dm)
+    n_out = 450000                                   # >= 148 window tiles, so AUTO keeps the window kernel
+    x = np.random.default_rng(5).standard_normal((2, n_out + int(tab.max()))).astype(np.float32)
+    got = plan.execute(to_dev(x), n_out).cpu().numpy()     # covered by the reserve above: no second reserve
+    assert plan.last_launches == 2 and plan.last_kernel == dd.KERNEL_WINDOW     # pairify + one band
+    ref, sa = oracle.brute_f32(x, tab, n_out)
+    check_f32(got, ref, sa)
+    plan.close()
+    torch.cuda.empty_cache()
+
+    cf = small_cfg("u8")
+    tab, x = make_case(oracle, cf, n_out=1000, beams=4)
+    plan = dd.Plan(**cf.plan_args())
+    plan.reserve(dd.U8, 100, 4)
+    plan.reserve(dd.U8, 1000, 1)
+    got = plan.execute(to_dev(x), 1000).cpu().numpy()
+    for b in range(4):
+        assert (got[b] == oracle.brute_u8(x[b], tab, 1000)).all()
+
+
+def test_last_kernel_reports_what_ran(oracle):
+    """dedisp_plan_last_kernel follows AUTO's size rule (dedisp_plan_resolved_kernel does not): cfg 1 has 15
+    register-window tiles for 148 SMs and runs one thread per output; the host entry judges the whole
+    buffer once, so its time pieces all run one kernel -- checked through the result being bit-identical
+    to the device entry's (same kernel, same fp32 summation order) on a buffer cut into pieces."""
+    cf = synth.configs()[1]
+    tab, x = make_case(oracle, cf)
+    plan = dd.Plan(**cf.plan_args())
+    assert plan.resolved_kernel(dd.F32) == dd.KERNEL_WINDOW and plan.last_kernel == -1
+    got = plan.execute(to_dev(x[0]), cf.n_out).cpu().numpy()
+    assert plan.last_kernel == dd.KERNEL_NAIVE
+    ref, sa = oracle.brute_f32(x[0], tab, cf.n_out)
+    check_f32(got, ref, sa)
+    # 64 trials x 70000 samples: 4 x 25 window tiles < 148 -> "small" as a whole; the host entry cuts it into
+    # 2 pieces (+ the split first one) which must not be judged one by one
+    cf2 = synth.scaled(cf, n_out=70000)
+    tab2, x2 = make_case(oracle, cf2)
+    p2 = dd.Plan(**cf2.plan_args())
+    dev = p2.execute(to_dev(x2[0]), cf2.n_out).cpu().numpy()
+    k = p2.last_kernel
+    assert k in (dd.KERNEL_NAIVE, dd.KERNEL_DIRECT)
+    host = p2.execute_host(x2[0], cf2.n_out)
+    assert p2.last_kernel == k and (np.asarray(host) == dev).all()
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_window_kernel_random_stress(oracle, seed):
+    """Randomised coverage of the register-window kernel's producer / consumer ring (the class of defect a
+    sanitizer would look for; compute-sanitizer is closed on this pool, profiles/r2_sanitizer.md): per seed a
+    random instantiated shape, band (cfg 2 / 3 / 5), channel count, DM step, DM offset and count, output
+    length from one sample to several blocks, 1-3 beams; uint8, so any lost, doubled or misplaced sample
+    changes an integer.  A shape whose ring does not fit the table falls back to the plan's own shape.  Run
+    twice on the same buffers: the second execute must reproduce the first bit for bit."""
+    rng = np.random.default_rng(7000 + seed)
+    T, G, NT, D = GEOMS[int(rng.integers(len(GEOMS)))]
+    base = synth.configs()[int(rng.choice([2, 3, 5]))]
+    nchans = int(rng.choice([33, 64, 200, 384, 1024]))
+    ndm = int(rng.integers(1, 3 * D * G + 1))
+    n_out = int(rng.integers(1, 5 * 2 * NT * 32 * T))
+    beams = int(rng.integers(1, 4))
+    step = float(base.dm_step * rng.choice([0.5, 1.0, 2.0]))
+    first = int(rng.integers(0, base.ndm))                 # where in the DM range the rows sit
+    dm = (first + np.arange(ndm)) * step
+    cf = synth.scaled(base, dtype="u8", n_out=n_out, ndm=ndm, nchans=nchans, dm_step=step, seed=100 + seed)
+    tab = oracle.shift_table(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, dm)
+    n_in = n_out + int(tab.max())
+    x = np.stack([synth.make_input(cf, n_in, beam=b) for b in range(beams)])
+    plan = dd.Plan(cf.nchans, cf.f_top_mhz, cf.df_mhz, cf.t_samp_ms, dm)
+    assert (plan.shifts() == tab).all()
+    try:
+        plan.set_window_geometry(T, G, NT, D)
+    except dd.DedispError as e:
+        assert e.status == dd.binding.ESTATE
+    info = plan.window_info()
+    if not info["ok"]:
+        pytest.skip("table outside the register-window kernel's limits for every shape")
+    plan.set_kernel(dd.KERNEL_WINDOW)
+    xd = to_dev(x)
+    got = plan.execute(xd, n_out).cpu().numpy()
+    assert plan.last_launches == 1 + info["nband"]
+    for b in range(beams):
+        assert (got[b] == oracle.brute_u8(x[b], tab, n_out)).all(), (seed, (T, G, NT, D), nchans, ndm, n_out, beams)
+    assert (plan.execute(xd, n_out).cpu().numpy() == got).all()
